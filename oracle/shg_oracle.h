@@ -1,0 +1,94 @@
+/*
+ * shg_oracle.h -- CPU reference ("oracle") for the split-step Fourier propagation of the coupled
+ * fundamental (FH, A1) and second-harmonic (SH, A2) envelopes of arxiv/paper_2410_04994 (cuSHG).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may build, link, import or call it.  It shares no
+ * source, header, table or constant generator with the CUDA path under paper_2410_04994_b200/.
+ *
+ * Plain C99, double precision throughout, its own brute-force DFT and iterative radix-2 FFT, no
+ * blocking / fusion / reordering beyond what the paper's algorithm states.  "P:n" below cites line n of
+ * /root/reference/PAPER.md; "G<k>" cites the reading of an ambiguous passage listed in DESIGN.md §3.
+ *
+ * What is pinned (tests/test_oracle_pins.py, all `-m "not gpu"`):
+ *   orc_fft2            vs orc_dft2_brute (the definition), Parseval, inverse(forward(x)) = x
+ *   linear half-step    vs the analytic Gaussian beam of P:95 (Eq. 5): profile, w(z), Gouy phase
+ *   absorption          vs exp(-alpha z)
+ *   coupling + RK4      vs power conservation, tanh^2 depletion, sinc^2 mismatch, Boyd-Kleinman h(sigma, xi)
+ *   TPA                 vs I0/(1+beta I0 z)
+ *   temperature/phase   vs sinc^2 with dk = dk0 + g dT for every nzt encoding of the same field,
+ *                       and the closed form for a linear-in-z mismatch
+ * The complete path with everything switched on at once (diffraction + coupling + T + TPA, the five
+ * BASELINE configs) has no closed form and no paper-printed value: for those runs "parity unpinned"
+ * beyond the component pins above and dz-refinement self-convergence.
+ */
+#ifndef SHG_ORACLE_H
+#define SHG_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_ctx orc_ctx;
+
+/* Transverse grid, z discretisation, temperature-plane count, batch capacity.  P:78. */
+typedef struct {
+    int32_t nx, ny;   /* transverse points, powers of two >= 2 (FFT grid, x fastest in memory)       */
+    int32_t nz;       /* z-steps >= 1, dz = L / nz                                          */
+    int32_t nzt;      /* temperature planes: 0 = uniform scalar, 1 = one plane for every z,
+                         >= 2 = planes at z_k = k L/(nzt-1), linear interpolation in z (G15)         */
+    int32_t batch;    /* independent simulations                                                      */
+} orc_grid;
+
+/* Crystal constants, SI.  P:72-76 (Eq. 2), P:80-84 (Eq. 3-4, linearised per north_star).          */
+typedef struct {
+    double L, lambda1, n1, n2, d_eff;
+    double dk0, ddk_dT, T_pm;      /* dk(T) = dk0 + ddk_dT (T - T_pm)   [rad/m, rad/(m K), K or C]   */
+    double alpha1, alpha2;         /* linear intensity absorption, 1/m                               */
+    double beta1, beta2;           /* two-photon absorption, m/W (G5)                                */
+} orc_crystal;
+
+/* Per-member beam / window.  P:95-104 (Eq. 5-6). P, w0, focus_z are used only by orc_gaussian_input. */
+typedef struct {
+    double P, w0, focus_z;         /* W, m (1/e field radius), m from the entrance face              */
+    double lx, ly;                 /* transverse window of this member, m; dx = lx / nx              */
+} orc_beam;
+
+/* Scheme switches (test aids; all 0 = the north_star path). */
+typedef struct {
+    int32_t scheme;      /* 0: L/2 - N(dz) - L/2 (north_star);  1: N/2 - L - N/2 (Eq. 14-15) */
+    int32_t undepleted;  /* 1: drop the coupling term of dA1/dz ("dPump = 0")                  */
+    int32_t brute_dft;   /* 1: use the O(N^2)-per-line DFT definition instead of the radix-2 FFT      */
+} orc_options;
+
+int  orc_create(const orc_grid*, const orc_crystal*, const orc_beam* beams /*[batch]*/,
+                const orc_options* opt /*NULL = defaults*/, orc_ctx** out);
+/* T: host fp32 [per_member ? batch : 1][nzt][ny][nx]; ignored (may be NULL) when nzt == 0, in which
+ * case every point has temperature T_uniform.  The array is borrowed until orc_propagate returns.  */
+int  orc_set_temperature(orc_ctx*, const float* T, double T_uniform, int per_member);
+/* Fields: host complex128 (interleaved re, im), [batch][ny][nx].  A2_in may be NULL (zeros).        */
+int  orc_propagate(orc_ctx*, const double* A1_in, const double* A2_in, double* A1_out, double* A2_out,
+                   int batch);
+/* Power (W) of both fields of one member at the recorded node nearest to z.  P:120 (I).      */
+int  orc_power(orc_ctx*, int member, double z, double* P1, double* P2);
+/* Whole history of one member: out[(nz+1)][2] = {P1(z_n), P2(z_n)}, n = 0..nz.                       */
+int  orc_power_history(orc_ctx*, int member, double* out);
+void orc_destroy(orc_ctx*);
+
+/* Gaussian input of P:104 (Eq. 6) generalised to any focus by P:95-100 (Eq. 5, tau0 = -focus_z/zR)
+ * with |A_F0|^2 = 4P/(eps0 c n1 pi w0^2) (G17).  out: complex128 [ny][nx] for member `member`.      */
+int  orc_gaussian_input(const orc_grid*, const orc_crystal*, const orc_beam* beam, double* out);
+
+/* Stand-alone transforms for the pins.  data: complex128 [ny][nx] interleaved.  sign = -1 forward
+ * (kernel e^{-i...}, unnormalised), +1 inverse (kernel e^{+i...}, divided by nx*ny).  P:340 (Eq. A.2). */
+int  orc_fft2(double* data, int ny, int nx, int sign);
+int  orc_dft2_brute(const double* in, double* out, int ny, int nx, int sign);
+
+int  orc_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
