@@ -1,0 +1,138 @@
+/*
+ * shg.h -- C ABI of libshg: B200-native (sm_100a) split-step Fourier propagation of the coupled
+ * fundamental (FH, A1) and second-harmonic (SH, A2) slowly-varying envelopes through a chi(2) crystal,
+ * the computation that dominates cuSHG (arxiv/paper_2410_04994).
+ *
+ * "P:n" cites line n of the paper text; "G<k>" a reading listed in DESIGN.md §3.
+ *
+ * What one call to shg_propagate computes, per batch member (members are independent):
+ *   for n = 0 .. nz-1:                                  dz = L/nz
+ *     A_j <- F^-1{ exp(-i(kx^2+ky^2)(dz/2)/(2k_j) - alpha_j dz/4) F{A_j} }, j = 1,2    (G3)
+ *     one classical RK4 step of length dz, independently at every (x,y), of              (Eq. 2, G2, G5)
+ *        dA1/dz = i kappa1 A2 conj(A1) e^{-i phi} - (beta1/2) I1 A1
+ *        dA2/dz = i kappa2 A1^2        e^{+i phi} - (beta2/2) I2 A2,   I_j = eps0 c n_j |A_j|^2 / 2
+ *        phi(x,y,z) = int_0^z dk dz',  dk = dk0 + ddk_dT (T(x,y,z) - T_pm)                (Eq. 3; north_star)
+ *     the same linear half-step again                                                     (order L/2-N-L/2)
+ *     P_j(z_{n+1}) = (eps0 c n_j / 2) dx dy sum |A_j|^2
+ *   (the two half-steps of neighbouring z-steps are applied as one full step; this is exact.)
+ *
+ * Conventions
+ *   - SI units.  Fields are complex fp32, interleaved (re, im), layout [batch][ny][nx], x fastest.
+ *     Grid point (iy, ix) sits at x = (ix - nx/2) lx/nx, y = (iy - ny/2) ly/ny (periodic FFT grid, G11).
+ *   - Every pointer argument says HOST or DEVICE.  Device pointers must be 16-byte aligned and belong to
+ *     the current CUDA device; the caller owns them.  The library owns its tables, the phase accumulator
+ *     phi, the power history and staging buffers, all allocated in shg_create / shg_set_temperature_host
+ *     and freed in shg_destroy; shg_propagate allocates nothing.
+ *   - shg_propagate enqueues work on the given stream and returns without waiting.  shg_power and
+ *     shg_power_history synchronise that stream.
+ *   - Every call returns SHG_OK (0) or a negative code; nothing aborts or throws across the ABI.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one returns SHG_ECUDA.
+ */
+#ifndef SHG_H
+#define SHG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SHG_OK       0
+#define SHG_EINVAL  (-1)   /* NULL / out-of-range argument, unsupported grid size                     */
+#define SHG_ESTATE  (-2)   /* call made in the wrong state (temperature not set, power before run)   */
+#define SHG_ECUDA   (-3)   /* a CUDA call failed; shg_strerror(SHG_ECUDA) carries the CUDA message    */
+#define SHG_ENOMEM  (-4)   /* host or device allocation failed                                        */
+
+typedef struct shg_ctx shg_ctx;   /* opaque, owned by the library */
+
+/* Transverse grid, z discretisation, temperature planes, batch capacity. */
+typedef struct {
+    int32_t nx, ny;   /* powers of two in {64,128,256,512,1024}; nx != ny is allowed                 */
+    int32_t nz;       /* z-steps >= 1                                                                */
+    int32_t nzt;      /* temperature planes: 0 = uniform scalar; 1 = one plane used at every z;
+                         >= 2 = planes at z_k = k L/(nzt-1), linearly interpolated to the step nodes
+                         z_n = n dz: s = n (nzt-1)/nz, k = min(floor(s), nzt-2), T = (1-f)T[k] + f T[k+1] (G15) */
+    int32_t batch;    /* capacity: number of independent simulations one propagate may carry         */
+} shg_grid;
+
+/* Crystal constants (Eq. 2; Eq. 3-4 in the linearised form the north_star fixes). */
+typedef struct {
+    double L, lambda1, n1, n2, d_eff;   /* m, m (FH vacuum wavelength; SH is lambda1/2), -, -, m/V    */
+    double dk0, ddk_dT, T_pm;           /* rad/m, rad/(m K), same unit as T                           */
+    double alpha1, alpha2;              /* linear intensity absorption, 1/m                           */
+    double beta1, beta2;                /* two-photon absorption, m/W                                 */
+} shg_crystal;
+
+/* One batch member's beam and transverse window (Eq. 5-6). */
+typedef struct {
+    double P, w0, focus_z;   /* W; m, 1/e field radius at the waist; focus distance from the entrance face, m.
+                                Used only by shg_gaussian_input.                                       */
+    double lx, ly;           /* transverse window, m (dx = lx/nx).  Members may differ (parameter sweeps). */
+} shg_beam;
+
+/* Options for shg_set_option. */
+#define SHG_OPT_PERSISTENT 1   /* 1 (default): one persistent cooperative kernel runs the whole z-loop with
+                                  device-wide barriers between the row and column passes (square grids);
+                                  0: two ordinary kernel launches per z-step (any nx, ny).              */
+#define SHG_OPT_PRECISE    2   /* 1 (default): every reused constant (FFT twiddles, propagator tables) is an
+                                  fp32 hi+lo pair whose lo part enters the FMA addend, so constant rounding
+                                  does not accumulate linearly over thousands of z-steps; 0: plain fp32.  */
+
+/* beams: HOST array [grid->batch].  *out receives the context. */
+int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);
+
+int shg_set_option(shg_ctx* ctx, int option, int value);
+
+/* Temperature field.  nzt == 0: T is ignored (may be NULL) and every point has temperature T_uniform.
+ * nzt >= 1: T is a DEVICE fp32 array [per_member ? batch : 1][nzt][ny][nx]; it is BORROWED (not copied)
+ * and must stay valid and unchanged until every propagate that uses it has completed. */
+int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, int per_member);
+
+/* Same, from a HOST array: copied (asynchronously on `cuda_stream` when the memory is pinned) into a
+ * library-owned device buffer that is allocated on first use and reused afterwards. */
+int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform, int per_member,
+                             void* cuda_stream);
+
+/* Propagate `batch` (<= capacity) members from z = 0 to z = L.
+ * A1_in, A2_in, A1_out, A2_out: DEVICE complex fp32 [batch][ny][nx].  A2_in may be NULL (zeros: the
+ * configs' A_SH(0) = 0).  In-place (A1_out == A1_in and/or A2_out == A2_in) is allowed; A1_out and
+ * A2_out must not overlap each other.  The outputs are also the kernels' working storage.
+ * cuda_stream: a cudaStream_t (NULL = the legacy default stream). */
+int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out,
+                  int batch, void* cuda_stream);
+
+/* Same with HOST buffers (pinned memory makes the copies asynchronous): copies the inputs to
+ * library-owned device buffers, propagates, copies both outputs back, all on `cuda_stream`.  Returns
+ * after enqueueing; synchronise the stream (or call shg_power) before reading the outputs. */
+int shg_propagate_host(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out,
+                       int batch, void* cuda_stream);
+
+/* Power (W) of both fields of `member` at the recorded node nearest to z (nodes z_n = n L/nz, n = 0..nz).
+ * The SH efficiency is derived by the caller: eta = P2(L) / (P1(0) + P2(0))  (G16). */
+int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2);
+
+/* Whole history of `member`: out is a HOST array [nz+1][2] = {P1(z_n), P2(z_n)}. */
+int shg_power_history(shg_ctx* ctx, int member, double* out);
+
+/* Fill A1 (DEVICE complex fp32 [batch][ny][nx]) with the Gaussian pump of Eq. 6 / Eq. 5 of every
+ * member's beam: A = A0/(1+i tau0) exp(-(x^2+y^2)/(w0^2 (1+i tau0))), tau0 = -focus_z/zR, zR = k1 w0^2/2,
+ * |A0|^2 = 4P/(eps0 c n1 pi w0^2) (G17). */
+int shg_gaussian_input(shg_ctx* ctx, void* A1_device, int batch, void* cuda_stream);
+
+/* Device timing of the z-loop: with timing enabled, shg_propagate records CUDA events on its stream right
+ * before and after the main-loop kernel(s) (the persistent kernel, or the 2 nz per-pass launches); the
+ * opening / closing half-step launches are outside.  shg_last_main_loop_ms synchronises the stream. */
+int shg_enable_timing(shg_ctx* ctx, int on);
+int shg_last_main_loop_ms(shg_ctx* ctx, float* ms);
+
+/* Number of kernels the last shg_propagate / shg_propagate_host launched. */
+int shg_last_launch_count(const shg_ctx* ctx);
+
+void shg_destroy(shg_ctx* ctx);
+
+const char* shg_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

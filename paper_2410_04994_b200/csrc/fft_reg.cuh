@@ -1,0 +1,149 @@
+// fft_reg.cuh -- register-resident radix-R complex FFTs (R = 2..32) and the hi+lo constant multiply.
+//
+// Everything here is compile-time indexed (templates + fold expressions), so the R complex values of a
+// thread live in registers and every internal twiddle is an immediate.
+//
+// Why hi+lo constants: the SSFM applies the SAME transform and propagator thousands of times, so an
+// fp32-rounded constant is a FIXED perturbation of the per-step operator and its error grows linearly
+// with the step count.  Each reused constant w is held as W = fl32(w), w' = fl32(w - W)
+// and the small product v*w' is put in the FMA ADDEND of the large one, so it is added before the large
+// product is rounded:  v*w ~= fma(v, W, v*w').  (fl(v*W) + fl(v*w') as two rounded products would discard it.)
+#pragma once
+
+#include <cuda_runtime.h>
+#include <utility>
+
+namespace shg {
+
+// cos(2 pi e / 32), e = 0..8, to 20 digits.
+__host__ __device__ constexpr double cos32_table(int e) {
+    constexpr double t[9] = {1.0,
+                             0.98078528040323044913,
+                             0.92387953251128675613,
+                             0.83146961230254523708,
+                             0.70710678118654752440,
+                             0.55557023301960222474,
+                             0.38268343236508977173,
+                             0.19509032201612826785,
+                             0.0};
+    return t[e];
+}
+// cos / sin of 2 pi e / 32 for e = 0..15
+__host__ __device__ constexpr double cos32(int e) { return e <= 8 ? cos32_table(e) : -cos32_table(16 - e); }
+__host__ __device__ constexpr double sin32(int e) { return e <= 8 ? cos32_table(8 - e) : cos32_table(e - 8); }
+
+__host__ __device__ constexpr float hi_of(double x) { return (float)x; }
+__host__ __device__ constexpr float lo_of(double x) { return (float)(x - (double)(float)x); }
+
+// t * c for a compile-time real constant c = C + c'
+template <bool PREC>
+__device__ __forceinline__ float mul_const(float t, float C, float c_lo) {
+    if constexpr (PREC) return fmaf(t, C, t * c_lo);
+    else return t * C;
+}
+
+// v * (W + w') for a complex constant; w4 = (W.re, W.im, w'.re, w'.im).  CONJ multiplies by conj(w).
+template <bool CONJ, bool PREC>
+__device__ __forceinline__ float2 cmul_hl(float2 v, float Wr, float Wi, float wr, float wi) {
+    float2 r;
+    if constexpr (!CONJ) {
+        if constexpr (PREC) {
+            r.x = fmaf(v.x, Wr, fmaf(-v.y, Wi, fmaf(v.x, wr, -v.y * wi)));
+            r.y = fmaf(v.x, Wi, fmaf(v.y, Wr, fmaf(v.x, wi, v.y * wr)));
+        } else {
+            r.x = fmaf(v.x, Wr, -v.y * Wi);
+            r.y = fmaf(v.x, Wi, v.y * Wr);
+        }
+    } else {
+        if constexpr (PREC) {
+            r.x = fmaf(v.x, Wr, fmaf(v.y, Wi, fmaf(v.x, wr, v.y * wi)));
+            r.y = fmaf(v.y, Wr, fmaf(-v.x, Wi, fmaf(v.y, wr, -v.x * wi)));
+        } else {
+            r.x = fmaf(v.x, Wr, v.y * Wi);
+            r.y = fmaf(v.y, Wr, -v.x * Wi);
+        }
+    }
+    return r;
+}
+
+template <bool CONJ, bool PREC>
+__device__ __forceinline__ float2 cmul_hl(float2 v, float4 w) {
+    return cmul_hl<CONJ, PREC>(v, w.x, w.y, w.z, w.w);
+}
+
+// d * exp(-/+ 2 pi i E / 32)   (INV: + sign), E = 0..15 compile time
+template <int E, bool INV, bool PREC>
+__device__ __forceinline__ float2 twmul32(float2 d) {
+    if constexpr (E == 0) {
+        return d;
+    } else if constexpr (E == 8) {           // -i (fwd) / +i (inv)
+        return INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);
+    } else if constexpr (E == 4) {           // (1 -/+ i)/sqrt2
+        constexpr float C = hi_of(cos32(4)), c = lo_of(cos32(4));
+        float a = INV ? d.x - d.y : d.x + d.y;
+        float b = INV ? d.x + d.y : d.y - d.x;
+        return make_float2(mul_const<PREC>(a, C, c), mul_const<PREC>(b, C, c));
+    } else if constexpr (E == 12) {          // (-1 -/+ i)/sqrt2
+        constexpr float C = hi_of(cos32(4)), c = lo_of(cos32(4));
+        float a = INV ? -(d.x + d.y) : d.y - d.x;
+        float b = INV ? d.x - d.y : -(d.x + d.y);
+        return make_float2(mul_const<PREC>(a, C, c), mul_const<PREC>(b, C, c));
+    } else {
+        // w = cos - i sin (fwd); conj for inverse
+        constexpr float Wr = hi_of(cos32(E)), wr = lo_of(cos32(E));
+        constexpr float Wi = hi_of(-sin32(E)), wi = lo_of(-sin32(E));
+        return cmul_hl<INV, PREC>(d, Wr, Wi, wr, wi);
+    }
+}
+
+// one decimation-in-frequency butterfly of span SPAN: (a, b) -> (a + b, (a - b) w)
+template <int R, int SPAN, int J, bool INV, bool PREC>
+__device__ __forceinline__ void dif_bfly(float2 (&v)[R]) {
+    constexpr int grp = J / SPAN, k = J % SPAN;
+    constexpr int i0 = grp * 2 * SPAN + k, i1 = i0 + SPAN;
+    constexpr int E = k * (16 / SPAN);       // W_{2 SPAN}^k = W_32^{k 16/SPAN}
+    float2 a = v[i0], b = v[i1];
+    v[i0] = make_float2(a.x + b.x, a.y + b.y);
+    v[i1] = twmul32<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));
+}
+
+template <int R, int SPAN, bool INV, bool PREC, int... J>
+__device__ __forceinline__ void dif_stage(float2 (&v)[R], std::integer_sequence<int, J...>) {
+    (dif_bfly<R, SPAN, J, INV, PREC>(v), ...);
+}
+
+template <int R, int SPAN, bool INV, bool PREC>
+__device__ __forceinline__ void dif_stages(float2 (&v)[R]) {
+    if constexpr (SPAN >= 1) {
+        dif_stage<R, SPAN, INV, PREC>(v, std::make_integer_sequence<int, R / 2>{});
+        dif_stages<R, SPAN / 2, INV, PREC>(v);
+    }
+}
+
+__host__ __device__ constexpr int bitrev(int i, int n) {
+    int r = 0;
+    for (int b = 1; b < n; b <<= 1) { r = (r << 1) | (i & 1); i >>= 1; }
+    return r;
+}
+
+template <int R, int I>
+__device__ __forceinline__ void brev_swap(float2 (&v)[R]) {
+    constexpr int j = bitrev(I, R);
+    if constexpr (I < j) { float2 t = v[I]; v[I] = v[j]; v[j] = t; }
+}
+
+template <int R, int... I>
+__device__ __forceinline__ void brev_all(float2 (&v)[R], std::integer_sequence<int, I...>) {
+    (brev_swap<R, I>(v), ...);
+}
+
+// In-place length-R DFT of v[0..R-1], natural order in and out.
+//   forward: V[k] = sum_n v[n] e^{-2 pi i n k / R};  INV: e^{+...}, unnormalised.
+template <int R, bool INV, bool PREC>
+__device__ __forceinline__ void fft_reg(float2 (&v)[R]) {
+    static_assert(R == 2 || R == 4 || R == 8 || R == 16 || R == 32, "radix");
+    dif_stages<R, R / 2, INV, PREC>(v);
+    brev_all<R>(v, std::make_integer_sequence<int, R>{});
+}
+
+}  // namespace shg

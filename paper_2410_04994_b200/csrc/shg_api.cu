@@ -1,0 +1,518 @@
+// shg_api.cu -- host side of libshg: the C ABI of include/shg.h.  Builds the constant tables in fp64 and
+// splits them into fp32 hi+lo pairs, owns the device state, and enqueues the kernels of shg_device.cuh.
+// There is no CPU fallback: every entry point that computes needs a CUDA device.
+#include "../../include/shg.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "shg_launch.h"
+#include "shg_params.h"
+
+namespace {
+
+constexpr double PI = 3.14159265358979323846264338327950288;
+constexpr double EPS0 = 8.8541878128e-12;   // F/m
+constexpr double C0 = 299792458.0;          // m/s
+
+thread_local std::string g_cuda_msg = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* what) {
+    g_cuda_msg = std::string(what) + ": " + cudaGetErrorString(e);
+    return SHG_ECUDA;
+}
+#define CU(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+struct Launchers {
+    cudaError_t (*row)(const shg::Params&, int, int, int, bool, int, cudaStream_t);
+    cudaError_t (*col)(const shg::Params&, int, bool, int, cudaStream_t);
+    cudaError_t (*persist)(const shg::Params&, bool, int, cudaStream_t);
+    shg::LaunchInfo (*info)();
+};
+
+bool launchers_for(int n, Launchers* L) {
+    switch (n) {
+#define SHG_CASE(N)                                                                                         \
+    case N:                                                                                                 \
+        *L = Launchers{shg::launch_row_##N, shg::launch_col_##N, shg::launch_persist_##N, shg::launch_info_##N}; \
+        return true;
+        SHG_CASE(64)
+        SHG_CASE(128)
+        SHG_CASE(256)
+        SHG_CASE(512)
+        SHG_CASE(1024)
+#undef SHG_CASE
+        default:
+            return false;
+    }
+}
+
+float4 split4(double re, double im) {
+    float hr = (float)re, hi = (float)im;
+    return make_float4(hr, hi, (float)(re - (double)hr), (float)(im - (double)hi));
+}
+
+__global__ void k_gaussian(float2* A, const shg::GaussDev* gd, int nx, int ny, int batch) {
+    size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    size_t np = (size_t)nx * ny;
+    if (i >= np * batch) return;
+    int b = (int)(i / np);
+    size_t r = i - (size_t)b * np;
+    int iy = (int)(r / nx), ix = (int)(r - (size_t)iy * nx);
+    shg::GaussDev g = gd[b];
+    float x = (ix - nx / 2) * g.dx, y = (iy - ny / 2) * g.dy;
+    float r2 = x * x + y * y;
+    float er = -r2 * g.qr, ei = -r2 * g.qi;
+    float mag = expf(er), c, s;
+    sincosf(ei, &s, &c);
+    A[i] = make_float2(mag * (g.ar * c - g.ai * s), mag * (g.ar * s + g.ai * c));
+}
+
+}  // namespace
+
+struct shg_ctx {
+    shg_grid g{};
+    shg_crystal c{};
+    std::vector<shg_beam> beams;
+    int device = 0;
+    int sm_count = 0;
+    bool persistent = true;
+    bool precise = true;
+    bool tables_dirty = true;
+
+    Launchers Lx{}, Ly{};
+
+    // device state
+    float4* d_twx = nullptr;
+    float4* d_twy = nullptr;
+    float4* d_hx[2] = {nullptr, nullptr};
+    float4* d_hy[2] = {nullptr, nullptr};
+    shg::MemberDev* d_mem = nullptr;
+    shg::GaussDev* d_gauss = nullptr;
+    float* d_phi = nullptr;
+    double* d_hist = nullptr;
+    unsigned int* d_barrier = nullptr;   // [0] barrier counter, [1] status word
+    float* d_T_owned = nullptr;
+    size_t T_owned_bytes = 0;
+    float2* d_stage[2] = {nullptr, nullptr};
+
+    const float* d_T = nullptr;
+    double T_uniform = 0.0;
+    int T_per_member = 0;
+    bool T_set = false;
+
+    bool timing = false;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    bool ev_recorded = false;
+
+    cudaStream_t last_stream = nullptr;
+    int last_batch = 0;
+    int last_launches = 0;
+    bool hist_valid = false;
+    std::vector<double> hist_host;
+};
+
+namespace {
+
+size_t np_of(const shg_ctx* ctx) { return (size_t)ctx->g.nx * ctx->g.ny; }
+
+// Tables that depend on the crystal, the grid, each member's window and the uniform temperature.
+int upload_tables(shg_ctx* ctx) {
+    const shg_grid& g = ctx->g;
+    const shg_crystal& c = ctx->c;
+    const int B = g.batch;
+    const double dz = c.L / g.nz;
+    const double k[2] = {2.0 * PI * c.n1 / c.lambda1, 2.0 * PI * c.n2 / (0.5 * c.lambda1)};
+    const double alpha[2] = {c.alpha1, c.alpha2};
+    const double beta[2] = {c.beta1, c.beta2};
+    const double nj[2] = {c.n1, c.n2};
+    const bool prec = ctx->precise;
+    auto mk = [&](double re, double im) {
+        float4 w = split4(re, im);
+        if (!prec) { w.z = 0.f; w.w = 0.f; }
+        return w;
+    };
+
+    // inter-stage twiddles exp(-2 pi i e / N)
+    for (int axis = 0; axis < 2; ++axis) {
+        const int n = axis ? g.ny : g.nx;
+        std::vector<float4> tw(n);
+        for (int e = 0; e < n; ++e) {
+            double a = -2.0 * PI * (double)e / (double)n;
+            tw[e] = mk(std::cos(a), std::sin(a));
+        }
+        CU(cudaMemcpy(axis ? ctx->d_twy : ctx->d_twx, tw.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
+    }
+
+    // separable propagator: hx_j[m] = exp(-i kx_m^2 h/(2 k_j) - alpha_j h/4), same in y, times 1/(nx ny)
+    // in the y table (P:346-352 Eq. A.4-A.5; sign per G3).  h = dz (index 0) and dz/2 (index 1).
+    for (int hs = 0; hs < 2; ++hs) {
+        const double h = hs ? 0.5 * dz : dz;
+        for (int axis = 0; axis < 2; ++axis) {
+            const int n = axis ? g.ny : g.nx;
+            const double scale = axis ? 1.0 / ((double)g.nx * (double)g.ny) : 1.0;
+            std::vector<float4> tab((size_t)B * 2 * n);
+            for (int b = 0; b < B; ++b) {
+                const double len = axis ? ctx->beams[b].ly : ctx->beams[b].lx;
+                for (int f = 0; f < 2; ++f)
+                    for (int m = 0; m < n; ++m) {
+                        const int ms = (m < n / 2) ? m : m - n;
+                        const double kk = 2.0 * PI * (double)ms / len;
+                        const double ang = -kk * kk * h / (2.0 * k[f]);
+                        const double mag = std::exp(-0.25 * alpha[f] * h) * scale;
+                        tab[((size_t)b * 2 + f) * n + m] = mk(mag * std::cos(ang), mag * std::sin(ang));
+                    }
+            }
+            CU(cudaMemcpy(axis ? ctx->d_hy[hs] : ctx->d_hx[hs], tab.data(), sizeof(float4) * tab.size(),
+                          cudaMemcpyHostToDevice));
+        }
+    }
+
+    // per-member scalars
+    std::vector<shg::MemberDev> mem(B);
+    std::vector<shg::GaussDev> gs(B);
+    const double kappa1 = 2.0 * PI * c.d_eff / (c.n1 * c.lambda1);
+    const double kappa2 = 2.0 * PI * c.d_eff / (c.n2 * c.lambda1);     // P:73 with G2
+    for (int b = 0; b < B; ++b) {
+        shg::MemberDev& m = mem[b];
+        const shg_beam& bm = ctx->beams[b];
+        m.kap1dz = (float)(kappa1 * dz);
+        m.kap2dz = (float)(kappa2 * dz);
+        m.g1dz = (float)(0.5 * beta[0] * 0.5 * EPS0 * C0 * nj[0] * dz);
+        m.g2dz = (float)(0.5 * beta[1] * 0.5 * EPS0 * C0 * nj[1] * dz);
+        m.dz = (float)dz;
+        m.dzd = dz;
+        m.gT = (float)c.ddk_dT;
+        m.Tpm_hi = (float)c.T_pm;
+        m.Tpm_lo = (float)(c.T_pm - (double)m.Tpm_hi);
+        m.dk0 = (float)c.dk0;
+        m.dk_uniform = c.dk0 + c.ddk_dT * (ctx->T_uniform - c.T_pm);
+        const double dxdy = (bm.lx / g.nx) * (bm.ly / g.ny);
+        for (int f = 0; f < 2; ++f) {
+            m.pscale_in[f] = 0.5 * EPS0 * C0 * nj[f] * dxdy;
+            m.pscale_step[f] = std::exp(-0.5 * alpha[f] * dz) * m.pscale_in[f];
+        }
+        // Eq. 5 at z = 0: tau0 = -focus_z / zR; |A0|^2 = 4P/(eps0 c n1 pi w0^2) (G17)
+        shg::GaussDev& gd = gs[b];
+        if (bm.w0 > 0.0) {
+            const double zR = 0.5 * bm.w0 * bm.w0 * k[0];
+            const double tau0 = -bm.focus_z / zR;
+            const double A0 = std::sqrt(4.0 * bm.P / (EPS0 * C0 * c.n1 * PI * bm.w0 * bm.w0));
+            const double den = 1.0 + tau0 * tau0;
+            gd.ar = (float)(A0 / den);
+            gd.ai = (float)(-A0 * tau0 / den);
+            gd.qr = (float)(1.0 / (bm.w0 * bm.w0 * den));
+            gd.qi = (float)(-tau0 / (bm.w0 * bm.w0 * den));
+        } else {
+            gd.ar = gd.ai = gd.qr = gd.qi = 0.f;
+        }
+        gd.dx = (float)(bm.lx / g.nx);
+        gd.dy = (float)(bm.ly / g.ny);
+    }
+    CU(cudaMemcpy(ctx->d_mem, mem.data(), sizeof(shg::MemberDev) * B, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_gauss, gs.data(), sizeof(shg::GaussDev) * B, cudaMemcpyHostToDevice));
+    ctx->tables_dirty = false;
+    return SHG_OK;
+}
+
+void free_ctx(shg_ctx* ctx) {
+    if (!ctx) return;
+    cudaFree(ctx->d_twx);
+    cudaFree(ctx->d_twy);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(ctx->d_hx[i]);
+        cudaFree(ctx->d_hy[i]);
+        cudaFree(ctx->d_stage[i]);
+    }
+    cudaFree(ctx->d_mem);
+    cudaFree(ctx->d_gauss);
+    cudaFree(ctx->d_phi);
+    cudaFree(ctx->d_hist);
+    cudaFree(ctx->d_barrier);
+    cudaFree(ctx->d_T_owned);
+    for (int i = 0; i < 2; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+const char* shg_strerror(int code) {
+    switch (code) {
+        case SHG_OK: return "ok";
+        case SHG_EINVAL: return "invalid argument (NULL / out of range / unsupported grid size)";
+        case SHG_ESTATE: return "call made in the wrong state (temperature not set, or power requested before a propagate)";
+        case SHG_ECUDA: return g_cuda_msg.c_str();
+        case SHG_ENOMEM: return "allocation failed";
+        default: return "unknown error code";
+    }
+}
+
+int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out) {
+    if (!grid || !crystal || !beams || !out) return SHG_EINVAL;
+    *out = nullptr;
+    Launchers Lx, Ly;
+    if (!launchers_for(grid->nx, &Lx) || !launchers_for(grid->ny, &Ly)) return SHG_EINVAL;
+    if (grid->nz < 1 || grid->nzt < 0 || grid->batch < 1) return SHG_EINVAL;
+    if (!(crystal->L > 0) || !(crystal->lambda1 > 0) || !(crystal->n1 > 0) || !(crystal->n2 > 0)) return SHG_EINVAL;
+    for (int b = 0; b < grid->batch; ++b)
+        if (!(beams[b].lx > 0) || !(beams[b].ly > 0)) return SHG_EINVAL;
+    if ((long long)grid->batch * grid->ny > (1LL << 30)) return SHG_EINVAL;
+
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    shg_ctx* ctx = new (std::nothrow) shg_ctx();
+    if (!ctx) return SHG_ENOMEM;
+    ctx->g = *grid;
+    ctx->c = *crystal;
+    ctx->beams.assign(beams, beams + grid->batch);
+    ctx->Lx = Lx;
+    ctx->Ly = Ly;
+    ctx->device = dev;
+    ctx->T_uniform = crystal->T_pm;
+    ctx->T_set = (grid->nzt == 0);
+    cudaError_t e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaDeviceGetAttribute"); }
+
+    const int B = grid->batch;
+    const size_t np = (size_t)grid->nx * grid->ny;
+    bool ok = true;
+    auto alloc = [&](void** p, size_t bytes) {
+        if (!ok) return;
+        cudaError_t e2 = cudaMalloc(p, bytes);
+        if (e2 != cudaSuccess) { ok = false; cuda_fail(e2, "cudaMalloc"); }
+    };
+    alloc((void**)&ctx->d_twx, sizeof(float4) * grid->nx);
+    alloc((void**)&ctx->d_twy, sizeof(float4) * grid->ny);
+    for (int hs = 0; hs < 2; ++hs) {
+        alloc((void**)&ctx->d_hx[hs], sizeof(float4) * (size_t)B * 2 * grid->nx);
+        alloc((void**)&ctx->d_hy[hs], sizeof(float4) * (size_t)B * 2 * grid->ny);
+    }
+    alloc((void**)&ctx->d_mem, sizeof(shg::MemberDev) * B);
+    alloc((void**)&ctx->d_gauss, sizeof(shg::GaussDev) * B);
+    if (grid->nzt > 0) alloc((void**)&ctx->d_phi, sizeof(float) * (size_t)B * np);
+    alloc((void**)&ctx->d_hist, sizeof(double) * (size_t)B * (grid->nz + 1) * 2);
+    alloc((void**)&ctx->d_barrier, 2 * sizeof(unsigned int));
+    if (!ok) { free_ctx(ctx); return SHG_ECUDA; }
+    ctx->hist_host.assign((size_t)B * (grid->nz + 1) * 2, 0.0);
+    int rc = upload_tables(ctx);
+    if (rc != SHG_OK) { free_ctx(ctx); return rc; }
+    *out = ctx;
+    return SHG_OK;
+}
+
+void shg_destroy(shg_ctx* ctx) { free_ctx(ctx); }
+
+int shg_set_option(shg_ctx* ctx, int option, int value) {
+    if (!ctx) return SHG_EINVAL;
+    switch (option) {
+        case SHG_OPT_PERSISTENT: ctx->persistent = (value != 0); return SHG_OK;
+        case SHG_OPT_PRECISE:
+            if (ctx->precise != (value != 0)) { ctx->precise = (value != 0); ctx->tables_dirty = true; }
+            return SHG_OK;
+        default: return SHG_EINVAL;
+    }
+}
+
+int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, int per_member) {
+    if (!ctx) return SHG_EINVAL;
+    if (ctx->g.nzt > 0 && (!T_device || !aligned16(T_device))) return SHG_EINVAL;
+    ctx->d_T = (ctx->g.nzt > 0) ? T_device : nullptr;
+    ctx->T_per_member = per_member ? 1 : 0;
+    if (ctx->T_uniform != T_uniform) { ctx->T_uniform = T_uniform; ctx->tables_dirty = true; }
+    ctx->T_set = true;
+    return SHG_OK;
+}
+
+int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform, int per_member,
+                             void* cuda_stream) {
+    if (!ctx) return SHG_EINVAL;
+    if (ctx->g.nzt == 0) return shg_set_temperature(ctx, nullptr, T_uniform, per_member);
+    if (!T_host) return SHG_EINVAL;
+    const size_t bytes = sizeof(float) * (size_t)(per_member ? ctx->g.batch : 1) * ctx->g.nzt * np_of(ctx);
+    if (ctx->T_owned_bytes < bytes) {
+        cudaFree(ctx->d_T_owned);
+        ctx->d_T_owned = nullptr;
+        ctx->T_owned_bytes = 0;
+        CU(cudaMalloc((void**)&ctx->d_T_owned, bytes));
+        ctx->T_owned_bytes = bytes;
+    }
+    CU(cudaMemcpyAsync(ctx->d_T_owned, T_host, bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+    return shg_set_temperature(ctx, ctx->d_T_owned, T_uniform, per_member);
+}
+
+int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out, int batch,
+                  void* cuda_stream) {
+    if (!ctx || !A1_in || !A1_out || !A2_out) return SHG_EINVAL;
+    if (batch < 1 || batch > ctx->g.batch) return SHG_EINVAL;
+    if (!aligned16(A1_in) || !aligned16(A2_in) || !aligned16(A1_out) || !aligned16(A2_out)) return SHG_EINVAL;
+    if (A1_out == A2_out) return SHG_EINVAL;
+    if (!ctx->T_set) return SHG_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (ctx->tables_dirty) {
+        // tables are uploaded with synchronous copies; make sure no earlier propagate still reads them
+        CU(cudaStreamSynchronize(ctx->last_stream));
+        int rc = upload_tables(ctx);
+        if (rc != SHG_OK) return rc;
+    }
+    const shg_grid& g = ctx->g;
+    shg::Params P{};
+    P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.nzt = g.nzt; P.batch = batch;
+    P.A[0] = (float2*)A1_out; P.A[1] = (float2*)A2_out;
+    P.Ain[0] = (const float2*)A1_in; P.Ain[1] = (const float2*)A2_in;
+    P.T = ctx->d_T; P.T_per_member = ctx->T_per_member;
+    P.phi = ctx->d_phi;
+    P.twx = ctx->d_twx; P.twy = ctx->d_twy;
+    for (int hs = 0; hs < 2; ++hs) { P.hx[hs] = ctx->d_hx[hs]; P.hy[hs] = ctx->d_hy[hs]; }
+    P.mem = ctx->d_mem;
+    P.hist = ctx->d_hist;
+    P.barrier = ctx->d_barrier;
+    P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
+
+    const size_t np = np_of(ctx);
+    CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(double) * (size_t)g.batch * (g.nz + 1) * 2, st));
+    CU(cudaMemsetAsync(ctx->d_barrier, 0, 2 * sizeof(unsigned int), st));
+    if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
+
+    const shg::LaunchInfo ix = ctx->Lx.info(), iy = ctx->Ly.info();
+    const int UR = batch * g.ny / ix.lines_per_warp;
+    const int UC = batch * 2 * g.nx / iy.cols_per_unit;
+    const int grid_r = UR < ctx->sm_count ? UR : ctx->sm_count;
+    const int grid_c = UC < ctx->sm_count ? UC : ctx->sm_count;
+    const bool prec = ctx->precise;
+    int launches = 0;
+
+    // opening half-step (x part) on the input, then its y part
+    CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 1, prec, grid_r, st)); ++launches;
+    CU(ctx->Ly.col(P, 1, prec, grid_c, st)); ++launches;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
+    if (ctx->persistent && g.nx == g.ny) {
+        const int grid_p = grid_r > grid_c ? grid_r : grid_c;
+        CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
+    } else {
+        for (int n = 0; n < g.nz; ++n) {
+            const int hsel = (n == g.nz - 1) ? 1 : 0;
+            CU(ctx->Lx.row(P, shg::ROW_MID, n, hsel, prec, grid_r, st)); ++launches;
+            CU(ctx->Ly.col(P, hsel, prec, grid_c, st)); ++launches;
+        }
+    }
+    if (ctx->timing) { CU(cudaEventRecord(ctx->ev[1], st)); ctx->ev_recorded = true; }
+    CU(ctx->Lx.row(P, shg::ROW_FINAL, 0, 0, prec, grid_r, st)); ++launches;
+
+    ctx->last_stream = st;
+    ctx->last_batch = batch;
+    ctx->last_launches = launches;
+    ctx->hist_valid = false;
+    return SHG_OK;
+}
+
+int shg_propagate_host(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out, int batch,
+                       void* cuda_stream) {
+    if (!ctx || !A1_in || !A1_out || !A2_out) return SHG_EINVAL;
+    if (batch < 1 || batch > ctx->g.batch) return SHG_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t cap = sizeof(float2) * (size_t)ctx->g.batch * np_of(ctx);
+    const size_t bytes = sizeof(float2) * (size_t)batch * np_of(ctx);
+    for (int i = 0; i < 2; ++i)
+        if (!ctx->d_stage[i]) CU(cudaMalloc((void**)&ctx->d_stage[i], cap));
+    CU(cudaMemcpyAsync(ctx->d_stage[0], A1_in, bytes, cudaMemcpyHostToDevice, st));
+    if (A2_in) CU(cudaMemcpyAsync(ctx->d_stage[1], A2_in, bytes, cudaMemcpyHostToDevice, st));
+    int rc = shg_propagate(ctx, ctx->d_stage[0], A2_in ? ctx->d_stage[1] : nullptr, ctx->d_stage[0], ctx->d_stage[1],
+                           batch, cuda_stream);
+    if (rc != SHG_OK) return rc;
+    CU(cudaMemcpyAsync(A1_out, ctx->d_stage[0], bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(A2_out, ctx->d_stage[1], bytes, cudaMemcpyDeviceToHost, st));
+    return SHG_OK;
+}
+
+static int fetch_history(shg_ctx* ctx) {
+    if (ctx->last_batch == 0) return SHG_ESTATE;
+    if (ctx->hist_valid) return SHG_OK;
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    unsigned int bs[2] = {0, 0};
+    CU(cudaMemcpy(bs, ctx->d_barrier, sizeof(bs), cudaMemcpyDeviceToHost));
+    if (bs[1] != 0) {
+        g_cuda_msg = "persistent kernel: device-wide barrier timed out (not all CTAs were co-resident?)";
+        return SHG_ECUDA;
+    }
+    CU(cudaMemcpy(ctx->hist_host.data(), ctx->d_hist, sizeof(double) * ctx->hist_host.size(), cudaMemcpyDeviceToHost));
+    ctx->hist_valid = true;
+    return SHG_OK;
+}
+
+int shg_power_history(shg_ctx* ctx, int member, double* out) {
+    if (!ctx || !out || member < 0 || member >= ctx->g.batch) return SHG_EINVAL;
+    int rc = fetch_history(ctx);
+    if (rc != SHG_OK) return rc;
+    if (member >= ctx->last_batch) return SHG_ESTATE;
+    const size_t n = (size_t)(ctx->g.nz + 1) * 2;
+    std::memcpy(out, ctx->hist_host.data() + (size_t)member * n, sizeof(double) * n);
+    return SHG_OK;
+}
+
+int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2) {
+    if (!ctx || !P1 || !P2 || member < 0 || member >= ctx->g.batch) return SHG_EINVAL;
+    int rc = fetch_history(ctx);
+    if (rc != SHG_OK) return rc;
+    if (member >= ctx->last_batch) return SHG_ESTATE;
+    const double dz = ctx->c.L / ctx->g.nz;
+    long n = std::lround(z / dz);
+    if (n < 0) n = 0;
+    if (n > ctx->g.nz) n = ctx->g.nz;
+    const double* h = ctx->hist_host.data() + (size_t)member * (ctx->g.nz + 1) * 2;
+    *P1 = h[2 * n];
+    *P2 = h[2 * n + 1];
+    return SHG_OK;
+}
+
+int shg_gaussian_input(shg_ctx* ctx, void* A1_device, int batch, void* cuda_stream) {
+    if (!ctx || !A1_device || batch < 1 || batch > ctx->g.batch) return SHG_EINVAL;
+    for (int b = 0; b < batch; ++b)
+        if (!(ctx->beams[b].w0 > 0) || !(ctx->beams[b].P >= 0)) return SHG_EINVAL;
+    if (ctx->tables_dirty) {
+        CU(cudaStreamSynchronize(ctx->last_stream));
+        int rc = upload_tables(ctx);
+        if (rc != SHG_OK) return rc;
+    }
+    const size_t total = np_of(ctx) * batch;
+    const int threads = 256;
+    const unsigned blocks = (unsigned)((total + threads - 1) / threads);
+    k_gaussian<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>((float2*)A1_device, ctx->d_gauss, ctx->g.nx,
+                                                                 ctx->g.ny, batch);
+    CU(cudaGetLastError());
+    return SHG_OK;
+}
+
+int shg_enable_timing(shg_ctx* ctx, int on) {
+    if (!ctx) return SHG_EINVAL;
+    if (on && !ctx->ev[0]) {
+        CU(cudaEventCreate(&ctx->ev[0]));
+        CU(cudaEventCreate(&ctx->ev[1]));
+    }
+    ctx->timing = (on != 0);
+    return SHG_OK;
+}
+
+int shg_last_main_loop_ms(shg_ctx* ctx, float* ms) {
+    if (!ctx || !ms) return SHG_EINVAL;
+    if (!ctx->ev_recorded) return SHG_ESTATE;
+    CU(cudaEventSynchronize(ctx->ev[1]));
+    CU(cudaEventElapsedTime(ms, ctx->ev[0], ctx->ev[1]));
+    return SHG_OK;
+}
+
+int shg_last_launch_count(const shg_ctx* ctx) { return ctx ? ctx->last_launches : SHG_EINVAL; }
+
+}  // extern "C"

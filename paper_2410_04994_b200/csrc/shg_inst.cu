@@ -1,0 +1,85 @@
+// shg_inst.cu -- kernel instantiations and launchers for one line length SHG_N (compiled once per N so the
+// sizes build in parallel).  Host code in shg_api.cu picks the launcher by nx / ny.
+#ifndef SHG_N
+#error "compile with -DSHG_N=<64|128|256|512|1024>"
+#endif
+
+#include "shg_device.cuh"
+#include "shg_launch.h"
+
+namespace shg {
+
+namespace {
+constexpr int N = SHG_N;
+using GE = Geo<N>;
+
+template <typename K>
+cudaError_t set_smem(K kernel, int bytes) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+template <int MODE, bool PREC>
+cudaError_t launch_row_t(const Params& P, int n, int hsel, int grid, cudaStream_t st) {
+    cudaError_t e = set_smem(k_row<N, MODE, PREC>, GE::CTA_SMEM);
+    if (e != cudaSuccess) return e;
+    k_row<N, MODE, PREC><<<grid, GE::THREADS, GE::CTA_SMEM, st>>>(P, n, hsel);
+    return cudaGetLastError();
+}
+
+template <bool PREC>
+cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
+    cudaError_t e = set_smem(k_col<N, PREC>, GE::CTA_SMEM);
+    if (e != cudaSuccess) return e;
+    k_col<N, PREC><<<grid, GE::THREADS, GE::CTA_SMEM, st>>>(P, hsel);
+    return cudaGetLastError();
+}
+
+template <bool PREC>
+cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
+    const int smem = GE::CTA_SMEM + N * (int)sizeof(float4);
+    cudaError_t e = set_smem(k_persist<N, PREC>, smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persist<N, PREC>, GE::THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    Params Pc = P;
+    void* args[] = {&Pc};
+    return cudaLaunchCooperativeKernel((const void*)k_persist<N, PREC>, dim3(grid), dim3(GE::THREADS), args,
+                                       (size_t)smem, st);
+}
+}  // namespace
+
+#define SHG_CAT_(a, b) a##b
+#define SHG_CAT(a, b) SHG_CAT_(a, b)
+
+cudaError_t SHG_CAT(launch_row_, SHG_N)(const Params& P, int mode, int n, int hsel, bool prec, int grid,
+                                        cudaStream_t st) {
+    if (prec) {
+        if (mode == ROW_FIRST) return launch_row_t<ROW_FIRST, true>(P, n, hsel, grid, st);
+        if (mode == ROW_MID) return launch_row_t<ROW_MID, true>(P, n, hsel, grid, st);
+        return launch_row_t<ROW_FINAL, true>(P, n, hsel, grid, st);
+    } else {
+        if (mode == ROW_FIRST) return launch_row_t<ROW_FIRST, false>(P, n, hsel, grid, st);
+        if (mode == ROW_MID) return launch_row_t<ROW_MID, false>(P, n, hsel, grid, st);
+        return launch_row_t<ROW_FINAL, false>(P, n, hsel, grid, st);
+    }
+}
+
+cudaError_t SHG_CAT(launch_col_, SHG_N)(const Params& P, int hsel, bool prec, int grid, cudaStream_t st) {
+    return prec ? launch_col_t<true>(P, hsel, grid, st) : launch_col_t<false>(P, hsel, grid, st);
+}
+
+cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid, cudaStream_t st) {
+    return prec ? launch_persist_t<true>(P, grid, st) : launch_persist_t<false>(P, grid, st);
+}
+
+LaunchInfo SHG_CAT(launch_info_, SHG_N)() {
+    LaunchInfo li;
+    li.lines_per_warp = GE::G;
+    li.cols_per_unit = GE::CW;
+    li.warps = GE::WARPS;
+    return li;
+}
+
+}  // namespace shg

@@ -1,0 +1,29 @@
+// shg_launch.h -- launcher prototypes shared by shg_inst.cu (one object per line length) and shg_api.cu.
+#pragma once
+
+#include <cuda_runtime.h>
+
+namespace shg {
+
+struct Params;
+
+struct LaunchInfo {
+    int lines_per_warp;   // G: rows per row-pass warp unit
+    int cols_per_unit;    // CW: columns per column-pass warp unit
+    int warps;            // warps per CTA
+};
+
+#define SHG_DECLARE_N(N)                                                                                   \
+    cudaError_t launch_row_##N(const Params& P, int mode, int n, int hsel, bool prec, int grid,            \
+                               cudaStream_t st);                                                            \
+    cudaError_t launch_col_##N(const Params& P, int hsel, bool prec, int grid, cudaStream_t st);           \
+    cudaError_t launch_persist_##N(const Params& P, bool prec, int grid, cudaStream_t st);                 \
+    LaunchInfo launch_info_##N();
+
+SHG_DECLARE_N(64)
+SHG_DECLARE_N(128)
+SHG_DECLARE_N(256)
+SHG_DECLARE_N(512)
+SHG_DECLARE_N(1024)
+
+}  // namespace shg

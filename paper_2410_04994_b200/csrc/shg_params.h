@@ -1,0 +1,45 @@
+// shg_params.h -- plain structs passed from the host side of libshg to its kernels.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace shg {
+
+// Per-member constants (device copy).  "P:n" = PAPER.md line n.
+struct MemberDev {
+    float kap1dz, kap2dz;      // kappa_j * dz                                   (P:72-73 with G2)
+    float g1dz, g2dz;          // (beta_j / 2) (eps0 c n_j / 2) dz                (G5)
+    float dz;
+    float gT;                  // ddk_dT
+    float Tpm_hi, Tpm_lo;      // T_pm = hi + lo
+    float dk0;
+    double dk_uniform;         // dk0 + ddk_dT (T_uniform - T_pm), used when nzt == 0
+    double dzd;
+    double pscale_in[2];       // (eps0 c n_j/2) dx dy
+    double pscale_step[2];     // exp(-alpha_j dz/2) (eps0 c n_j/2) dx dy  (Parseval: power after the closing half-step)
+};
+
+struct Params {
+    int nx, ny, nz, nzt, batch;
+    float2* A[2];              // working / output fields [batch][ny][nx]
+    const float2* Ain[2];      // inputs (Ain[1] may be null)
+    const float* T;            // [members][nzt][ny][nx] or null
+    int T_per_member;
+    float* phi;                // [batch][ny][nx]
+    const float4* twx;         // [nx]  exp(-2 pi i e/nx) as (hi.re, hi.im, lo.re, lo.im)
+    const float4* twy;         // [ny]
+    const float4* hx[2];       // [0]=full step dz, [1]=half step: [batch][2][nx]
+    const float4* hy[2];       // [batch][2][ny], includes 1/(nx ny)
+    const MemberDev* mem;      // [batch]
+    double* hist;              // [batch][nz+1][2]
+    unsigned int* barrier;     // grid barrier counter (persistent kernel)
+    int* status;               // device status word (barrier timeout)
+};
+
+enum RowMode { ROW_FIRST = 0, ROW_MID = 1, ROW_FINAL = 2 };
+
+// A0/(1+i tau0) and 1/(w0^2 (1+i tau0)) of one member, for the Gaussian pump of Eq. 5-6.
+struct GaussDev { float ar, ai, qr, qi, dx, dy; };
+
+}  // namespace shg

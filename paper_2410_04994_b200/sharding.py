@@ -1,0 +1,48 @@
+"""Multi-GPU plumbing.  Batch members are independent simulations (no exchange step anywhere in the
+path), so a sweep is sharded by member across ranks with NO data-path collective; the only communication
+is gathering the per-member efficiencies (a few doubles) at the end.  A single simulation does not shard
+(two all-to-all transposes per z-step over <= 16 MB of state would be latency bound): "replicas only".
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def member_range(n_members: int, rank: int, world: int) -> range:
+    """Contiguous, balanced split: the first (n_members % world) ranks get one extra member."""
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("bad rank/world")
+    base, extra = divmod(n_members, world)
+    lo = rank * base + min(rank, extra)
+    return range(lo, lo + base + (1 if rank < extra else 0))
+
+
+def shard_workload(w: dict, rank: int, world: int) -> dict:
+    """The slice of a batched workload (workloads.make output) that `rank` owns."""
+    r = member_range(w["grid"]["batch"], rank, world)
+    out = dict(w)
+    out["beams"] = [w["beams"][b] for b in r]
+    out["A1"] = w["A1"][r.start:r.stop]
+    out["grid"] = dict(w["grid"], batch=len(r))
+    if w.get("T") is not None and w.get("per_member"):
+        out["T"] = w["T"].reshape(w["grid"]["batch"], -1)[r.start:r.stop]
+    out["members"] = r
+    return out
+
+
+def gather_member_values(local: np.ndarray, n_members: int, rank: int, world: int, group=None) -> np.ndarray:
+    """All ranks receive the full per-member vector (e.g. the efficiency map of a sweep).
+    Uses torch.distributed (nccl or gloo) when world > 1; identity otherwise."""
+    local = np.asarray(local, dtype=np.float64)
+    if world == 1:
+        return local.copy()
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend(group) == "nccl" else "cpu"
+    sizes = [len(member_range(n_members, r, world)) for r in range(world)]
+    pad = max(sizes)
+    buf = torch.zeros(pad, dtype=torch.float64, device=dev)
+    buf[:len(local)] = torch.from_numpy(local).to(dev)
+    outs = [torch.zeros(pad, dtype=torch.float64, device=dev) for _ in range(world)]
+    dist.all_gather(outs, buf, group=group)
+    return np.concatenate([o[:s].cpu().numpy() for o, s in zip(outs, sizes)])

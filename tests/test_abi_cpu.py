@@ -1,0 +1,126 @@
+"""CPU-side checks of the product: the C-ABI library loads, exports every symbol include/shg.h declares,
+validates arguments, and refuses to compute without a CUDA device (no CPU fallback).  Plus the host logic
+of the multi-GPU sharding over gloo, world_size 2."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def shg_mod():
+    from paper_2410_04994_b200 import build, shg
+    build.build()
+    return shg
+
+
+def test_library_exports_every_declared_symbol(shg_mod):
+    header = open(os.path.join(ROOT, "include", "shg.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(shg_[a-z_0-9]+)\s*\(", header))
+    assert declared == set(shg_mod.EXPORTS)
+    L = shg_mod.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    out = subprocess.run(["nm", "-D", "--defined-only", shg_mod.LIB_PATH], capture_output=True, text=True).stdout
+    exported = set(re.findall(r" T (shg_[a-z_0-9]+)", out))
+    assert declared <= exported
+
+
+def test_argument_validation_and_no_cpu_fallback(shg_mod):
+    L = shg_mod.lib()
+    g = shg_mod.Grid(64, 64, 10, 0, 1)
+    c = shg_mod._mk(shg_mod.Crystal, dict(L=0.03, lambda1=1064e-9, n1=2.14, n2=2.18, d_eff=1e-11))
+    b = (shg_mod.Beam * 1)(shg_mod._mk(shg_mod.Beam, dict(P=1.0, w0=3e-5, focus_z=0.015, lx=2e-4, ly=2e-4)))
+    h = C.c_void_p()
+    assert L.shg_create(None, C.byref(c), b, C.byref(h)) == shg_mod.SHG_EINVAL
+    for bad in (dict(nx=48), dict(nx=2048), dict(ny=32), dict(nz=0), dict(nzt=-1), dict(batch=0)):
+        gg = shg_mod.Grid(64, 64, 10, 0, 1)
+        for k, v in bad.items():
+            setattr(gg, k, v)
+        assert L.shg_create(C.byref(gg), C.byref(c), b, C.byref(h)) == shg_mod.SHG_EINVAL, bad
+    cz = shg_mod._mk(shg_mod.Crystal, dict(L=0.0, lambda1=1064e-9, n1=2.14, n2=2.18))
+    assert L.shg_create(C.byref(g), C.byref(cz), b, C.byref(h)) == shg_mod.SHG_EINVAL
+    b0 = (shg_mod.Beam * 1)(shg_mod._mk(shg_mod.Beam, dict(lx=0.0, ly=1e-4)))
+    assert L.shg_create(C.byref(g), C.byref(c), b0, C.byref(h)) == shg_mod.SHG_EINVAL
+    assert L.shg_power(None, 0, 0.0, None, None) == shg_mod.SHG_EINVAL
+    assert L.shg_propagate(None, None, None, None, None, 1, None) == shg_mod.SHG_EINVAL
+    assert b"invalid argument" in L.shg_strerror(shg_mod.SHG_EINVAL)
+    import torch
+    if not torch.cuda.is_available():
+        # valid arguments, no device: the library must fail loudly, not fall back to the CPU
+        rc = L.shg_create(C.byref(g), C.byref(c), b, C.byref(h))
+        assert rc == shg_mod.SHG_ECUDA and not h.value
+        assert len(L.shg_strerror(rc)) > 0
+        with pytest.raises(shg_mod.ShgError):
+            shg_mod.Shg(dict(nx=64, ny=64, nz=10, nzt=0), dict(L=0.03, lambda1=1064e-9, n1=2.14, n2=2.18,
+                                                               d_eff=1e-11), [dict(lx=2e-4, ly=2e-4)])
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2410_04994_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.lower() or f == "workloads.py", f
+    # workloads.py mentions the oracle only in prose
+    src = open(os.path.join(pkg, "workloads.py")).read()
+    assert not re.search(r"^\s*(import|from)\s+oracle", src, flags=re.M)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            # prose may name the product package; no import, include or path into it
+            assert not re.search(r"^\s*(import|from)\s+paper_2410_04994_b200", src, flags=re.M), f
+            assert not re.search(r"#\s*include[^\n]*(paper_2410_04994_b200|csrc|shg\.h)", src), f
+            assert "libshg" not in src, f
+
+
+def test_member_range_is_a_balanced_partition():
+    from paper_2410_04994_b200.sharding import member_range
+    for n in (1, 7, 64, 65):
+        for world in (1, 2, 3, 8):
+            parts = [member_range(n, r, world) for r in range(world)]
+            assert [i for p in parts for i in p] == list(range(n))
+            sizes = [len(p) for p in parts]
+            assert max(sizes) - min(sizes) <= 1
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %(root)r)
+import numpy as np, torch, torch.distributed as dist
+from paper_2410_04994_b200 import workloads as wl
+from paper_2410_04994_b200.sharding import shard_workload, gather_member_values, member_range
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+w = wl.make("cfg4", nz=2, batch=7)
+mine = shard_workload(w, rank, world)
+assert mine["A1"].shape[0] == len(member_range(7, rank, world)) == mine["grid"]["batch"]
+# stand-in per-member result that identifies the member: its beam power
+local = np.array([b["P"] for b in mine["beams"]])
+full = gather_member_values(local, 7, rank, world)
+assert np.allclose(full, [b["P"] for b in w["beams"]]), full
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_two_rank_gloo_sharding_and_gather(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER % dict(root=ROOT))
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT="29731")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    for r, p in enumerate(procs):
+        out, _ = p.communicate(timeout=300)
+        assert p.returncode == 0 and ("ok %d" % r) in out, out
