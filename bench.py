@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py -- SSFM throughput of libshg on B200 (BASELINE.json metric: grid-point z-steps per second).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl reference]
+
+A "step" is one pass of the whole hot path over one workload: one shg_propagate (opening half-step, the nz
+fused z-steps, closing half-step, power history) of the named BASELINE.json config on synthetic seeded input.
+Prints ONE JSON line (rank 0).  See DESIGN.md §7 for what each key means and how the roofline numbers are
+formed.  `--impl reference` times the CPU oracle (oracle/, fp64, as it stands) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ssfm_grid_point_z_steps_per_s"
+UNIT = "pt-steps/s"
+NOMINAL_HBM_GBS = 8000.0            # the ~8 TB/s BASELINE.json names (context only)
+FALLBACK_HBM_GBS = 6650.0           # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# fp32 FMA peak for the "alu" side figure: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg5", help="cfg2 | cfg3 | cfg4 | cfg5 (default: the largest single-GPU config)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--nz", type=int, default=None, help="override the z-step count (profiling runs only; "
+                    "a number measured with --nz is not the config's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--per-pass", action="store_true", help="two launches per z-step instead of the persistent kernel")
+    return ap.parse_args()
+
+
+def measured_peak_hbm():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy kernel)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic_bytes(workload: str, nz: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed
+    ncu --set full summary (profiles/roofline_traffic.csv: workload,nz,kernel,dram_bytes_per_launch)."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = [s.strip() for s in line.split(",")]
+        if len(f) >= 4 and f[0] == workload and f[1].isdigit():
+            # scale linearly in the z-step count when the capture used a shorter run of the same kernel
+            return float(f[3]) * nz / int(f[1])
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.f = None
+        self.p = None
+
+    def start(self):
+        try:
+            self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+        return self
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw = [], [], []
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            c = [s.strip() for s in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            # "under load" = samples at or above the median (the sampler also sees the gaps between steps)
+            s = sorted(sm)
+            out.update(sm_mhz=s[len(s) // 2], sm_max_mhz=max(mx), power_w_max=max(pw), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle timing (reported baseline; the oracle as it stands, never tuned for this)
+# ------------------------------------------------------------------------------------------------
+def time_oracle_sample(w_full, budget_s: float, nz_probe: int = 1):
+    """Time oracle.propagate on a bounded sample of the workload: the same grid, crystal, beams, input field
+    and temperature array, but only `nz_s` z-steps (dz = L/nz_s), nz_s chosen from a 1-step probe so that the
+    run takes about `budget_s` seconds.  Returns (pt_steps_per_s, cores, description, seconds)."""
+    import numpy as np
+    import oracle
+    from paper_2410_04994_b200 import workloads as wl
+
+    g = w_full["grid"]
+    # members: a sweep is sampled by its first members (they are independent)
+    nb = min(g["batch"], 4)
+    npts = g["nx"] * g["ny"] * nb
+
+    def run(nz_s):
+        ws = wl.make(w_full["name"], nz=nz_s, batch=nb) if w_full["name"] == "cfg4" else \
+            (w_full if nz_s == g["nz"] else _with_nz(w_full, nz_s))
+        o = oracle.Oracle(ws["grid"], ws["crystal"], ws["beams"])
+        o.set_temperature(ws["T"], ws["T_uniform"], ws["per_member"])
+        a1 = ws["A1"].astype(np.complex128)
+        t0 = time.perf_counter()
+        o.propagate(a1)
+        dt = time.perf_counter() - t0
+        o.close()
+        return dt
+
+    t_probe = run(nz_probe)
+    per_step = max(t_probe / nz_probe, 1e-6)
+    nz_s = int(max(1, min(g["nz"], budget_s / per_step)))
+    dt = run(nz_s) if nz_s > nz_probe else t_probe
+    if nz_s <= nz_probe:
+        nz_s = nz_probe
+    desc = ("%s grid %dx%d, %d member(s), same input field and temperature array, rerun with "
+            "%d of %d z-steps (%.1f s)" % (w_full["name"], g["nx"], g["ny"], nb, nz_s, g["nz"], dt))
+    return npts * nz_s / dt, oracle.num_threads(), desc, dt
+
+
+def _with_nz(w, nz_s):
+    """Same workload with a different z-step count.  Configs whose T planes sit on the step nodes (nzt = nz+1)
+    are regenerated; a fixed-plane-count T (cfg5) is reused as is (it is interpolated in z)."""
+    from paper_2410_04994_b200 import workloads as wl
+    g = w["grid"]
+    if g["nzt"] == g["nz"] + 1:
+        return wl.make(w["name"], nz=nz_s)
+    out = dict(w)
+    out["grid"] = dict(g, nz=nz_s)
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config / metric / unit; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2410_04994_b200 import workloads as wl
+    import oracle
+    oracle.build()
+    w = wl.make(args.workload, nz=args.nz)
+    total = max(1, args.steps + args.warmup)
+    budget = min(20.0, 150.0 / total)          # whole run ends within a few minutes
+    vals, desc, cores = [], "", 1
+    for i in range(total):
+        v, cores, desc, dt = time_oracle_sample(w, budget)
+        if i >= args.warmup:
+            vals.append((v, dt))
+    value = sum(v for v, _ in vals) / len(vals)
+    g = w["grid"]
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(d for _, d in vals) / len(vals),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(w), "nx": g["nx"], "ny": g["ny"], "nz": g["nz"], "batch": g["batch"],
+                   "nzt": g["nzt"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_label(w):
+    labels = {"cfg1": "BASELINE.json configs[0]: 64x64, 200 z-steps",
+              "cfg2": "BASELINE.json configs[1]: 128x128, 1000 z-steps, absorption + T array",
+              "cfg3": "BASELINE.json configs[2]: 256x256, 4000 z-steps, T array",
+              "cfg4": "BASELINE.json configs[3]: 64 x (128x128, 1000 z-steps) parameter sweep",
+              "cfg5": "BASELINE.json configs[4]: 1024x1024, 10000 z-steps, 1 GiB T array"}
+    return labels.get(w["name"], w["name"])
+
+
+# ------------------------------------------------------------------------------------------------
+# B200 arm
+# ------------------------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2410_04994_b200 import shg
+    from paper_2410_04994_b200 import workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # Every rank runs one full replica of the workload (members / simulations are independent: no data-path
+    # collective; weak scaling).  DESIGN.md §8.
+    w = wl.make(args.workload, nz=args.nz)
+    g = w["grid"]
+    B = g["batch"]
+    pts = g["nx"] * g["ny"] * g["nz"] * B
+    ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=not args.per_pass)
+    ctx.enable_timing(True)
+    stream = torch.cuda.current_stream()
+
+    # ---- inputs resident in HBM
+    A1 = torch.from_numpy(w["A1"]).cuda()
+    Td = None
+    if g["nzt"] > 0:
+        Td = torch.from_numpy(w["T"]).cuda()
+        ctx.set_temperature(Td, per_member=w["per_member"])
+    else:
+        ctx.set_temperature(None, w["T_uniform"])
+    O1, O2 = torch.empty_like(A1), torch.empty_like(A1)
+
+    for _ in range(args.warmup):
+        ctx.propagate(A1, None, O1, O2)
+    barrier()
+    sampler = ClockSampler(local).start() if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record(stream)
+    for _ in range(args.steps):
+        ctx.propagate(A1, None, O1, O2)
+    ev[1].record(stream)
+    barrier()
+    ms_total = ev[0].elapsed_time(ev[1])
+    main_loop_ms = ctx.last_main_loop_ms()          # device time of the z-loop kernel(s) of the last step
+    launches = ctx.last_launch_count() * args.steps
+    clocks = sampler.stop() if sampler else None
+    eta = [ctx.efficiency(b) for b in range(B)]
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * pts / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry points: pinned host inputs -> device -> result on the host
+    e2e = None
+    if not args.no_e2e:
+        hA1 = torch.from_numpy(w["A1"]).pin_memory()
+        hO1, hO2 = torch.empty_like(hA1).pin_memory(), torch.empty_like(hA1).pin_memory()
+        hT = torch.from_numpy(w["T"]).pin_memory() if g["nzt"] > 0 else None
+        h2d = hA1.numel() * 8 + (hT.numel() * 4 if hT is not None else 0)
+        d2h = 2 * hA1.numel() * 8 + B * (g["nz"] + 1) * 2 * 8
+
+        def e2e_step():
+            if hT is not None:
+                ctx.set_temperature(hT, per_member=w["per_member"], stream=stream)
+            else:
+                ctx.set_temperature(None, w["T_uniform"])
+            ctx.propagate_host(hA1, None, hO1, hO2, stream=stream)
+            return ctx.power_history(0)            # synchronises the stream and reads the history back
+
+        for _ in range(max(1, min(args.warmup, 2))):
+            e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev2[0].record(stream)
+        for _ in range(args.steps):
+            e2e_step()
+        ev2[1].record(stream)
+        barrier()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        # host work (history read-back) sits between device work, so take the larger of the two clocks
+        ms_e2e = max(ev2[0].elapsed_time(ev2[1]), wall_ms)
+        t2 = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * pts / (float(t2.item()) / args.steps * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": float(t2.item()) / args.steps,
+               "api": "shg_set_temperature_host + shg_propagate_host + shg_power_history (pinned host buffers)"}
+        if g["nzt"] > 0:
+            ctx.set_temperature(Td, per_member=w["per_member"])
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (the z-loop kernel: k_persist, or the k_row/k_col pairs)
+    peak, peak_src = measured_peak_hbm()
+    b_alg = wl.algorithmic_bytes_per_point_step(w)
+    f_alg = wl.algorithmic_flops_per_point_step(w)
+    bytes_launch = b_alg * pts
+    achieved = bytes_launch / (main_loop_ms * 1e-3) / 1e9
+    traffic = ncu_traffic_bytes(w["name"], g["nz"])
+    roofline = {
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": traffic, "peak_source": peak_src,
+        "kernel": "k_persist<%d>" % g["nx"] if (not args.per_pass and g["nx"] == g["ny"]) else "k_row+k_col",
+        "kernel_ms_per_launch": main_loop_ms, "algorithmic_bytes_per_pt_step": b_alg,
+        "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+        "two_pass_traffic_GBs": (b_alg + 32.0) * pts / (main_loop_ms * 1e-3) / 1e9,
+        "alu": {"flops_per_pt_step": f_alg, "achieved_tflops": f_alg * pts / (main_loop_ms * 1e-3) / 1e12,
+                "fp32_peak_tflops_nominal": FP32_PEAK_TFLOPS,
+                "frac": f_alg * pts / (main_loop_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS},
+        "note": "fields (<= 16 MB) stay L2-resident across z-steps, so ncu dram bytes are below the algorithmic bytes",
+    }
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        import oracle
+        oracle.build()
+        v, cores, desc, dt = time_oracle_sample(w, 15.0)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_label(w), "nx": g["nx"], "ny": g["ny"], "nz": g["nz"], "batch": B,
+                   "nzt": g["nzt"], "launch": "per-pass" if args.per_pass else "persistent",
+                   "parallelism": "replicas x%d (no collective)" % world,
+                   "l2": "inputs larger than L2 where the config has a T array (cfg5: 1 GiB); the 16 MB field state "
+                         "is L2-resident by construction of the z-sequential method, no flush between steps"},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "eta_member0": eta[0],
+        "paper_context": "paper reports GPU/CPU speedup only: ~40x (17-43x), GTX 1650 vs i7-9700 (PAPER.md:13,272,312)",
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
