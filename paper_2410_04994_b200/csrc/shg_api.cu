@@ -141,14 +141,17 @@ int upload_tables(shg_ctx* ctx) {
         return w;
     };
 
-    // inter-stage twiddles exp(-2 pi i e / N)
+    // inter-stage twiddles W_N^{k1 m} = exp(-2 pi i k1 m / N), N = R M, stored [k1][m] so that the M lanes of a
+    // line read consecutive entries
     for (int axis = 0; axis < 2; ++axis) {
         const int n = axis ? g.ny : g.nx;
+        const shg::LaunchInfo li = axis ? ctx->Ly.info() : ctx->Lx.info();
         std::vector<float4> tw(n);
-        for (int e = 0; e < n; ++e) {
-            double a = -2.0 * PI * (double)e / (double)n;
-            tw[e] = mk(std::cos(a), std::sin(a));
-        }
+        for (int k1 = 0; k1 < li.fft_r; ++k1)
+            for (int m = 0; m < li.fft_m; ++m) {
+                double a = -2.0 * PI * (double)((long long)k1 * m % n) / (double)n;
+                tw[(size_t)k1 * li.fft_m + m] = mk(std::cos(a), std::sin(a));
+            }
         CU(cudaMemcpy(axis ? ctx->d_twy : ctx->d_twx, tw.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     }
 
@@ -387,8 +390,8 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
 
     const shg::LaunchInfo ix = ctx->Lx.info(), iy = ctx->Ly.info();
-    const int UR = batch * g.ny / ix.lines_per_warp;
-    const int UC = batch * 2 * g.nx / iy.cols_per_unit;
+    const int UR = batch * g.ny / ix.rows_per_item;          // row-pass items
+    const int UC = batch * 2 * (g.nx / iy.cols_per_item);    // column-pass strips
     const int grid_r = UR < ctx->sm_count ? UR : ctx->sm_count;
     const int grid_c = UC < ctx->sm_count ? UC : ctx->sm_count;
     const bool prec = ctx->precise;

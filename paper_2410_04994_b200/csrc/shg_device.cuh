@@ -1,14 +1,27 @@
-// shg_device.cuh -- device side of libshg: warp-autonomous 1-D FFTs, the fused row pass
-// (inverse FFT_x -> temperature/phase -> RK4 -> power -> forward FFT_x -> propagator) and column pass
-// (FFT_y -> propagator -> inverse FFT_y), the per-pass kernels and the persistent whole-run kernel.
+// shg_device.cuh -- device side of libshg: the warp-level 1-D FFT, the fused row pass
+// (FFT_x -> temperature/phase -> RK4 -> power -> FFT_x -> propagator) and column pass
+// (FFT_y -> propagator -> FFT_y), the per-pass kernels and the persistent whole-run kernel.
 //
-// Decomposition of one line of length N = R * M (R values per thread, M threads per line, G = 32/M lines
-// per warp):  n = M n1 + n2 (thread n2 = m holds n1 = 0..R-1),  k = k1 + R k2:
+// One line of length N = R * M is held by M lanes (R values per lane, G = 32/M lines per warp).
+// Decomposition  n = M n1 + n2 (lane n2 = m holds n1 = 0..R-1),  k = k1 + R k2:
 //   X[k1 + R k2] = sum_{n2} W_M^{n2 k2} [ W_N^{n2 k1} sum_{n1} W_R^{n1 k1} x[M n1 + n2] ]
 // stage A: radix-R in registers; twiddle W_N^{k1 m}; one transpose through shared memory (XOR-swizzled,
-// conflict free); stage B: R/M radix-M FFTs in registers.  Input and output are both in the "strided"
-// layout: thread m holds elements m + M q, q = 0..R-1 -- which is also the coalesced global layout.
-// A warp never synchronises with another warp inside a pass.
+// conflict free); stage B: R/M radix-M FFTs in registers.  Input and output are both "strided": lane m holds
+// elements m + M q, q = 0..R-1 -- which is also the coalesced global layout.
+//
+// Only the FORWARD transform exists in the code (one instance keeps the z-loop inside the instruction
+// cache).  Inverse transforms are taken as conj(F(conj(.))) with every conjugation folded into a neighbour:
+//   column pass:  F_y -> * hy, conjugated (free) -> F_y -> store            [global holds conj(field)]
+//   row pass:     load -> F_x -> conj (free, operand negation) -> RK4 -> F_x -> * hx -> store
+// so between a column pass and the next row pass global memory holds the complex conjugate of the field in
+// (k_x, y) representation.  DESIGN.md §5.
+//
+// The two fields of a row are transformed by different lane groups (or, at N = 1024, by the two warps of a
+// pair) and meet for the nonlinear step through shared memory.  To make the two sides symmetric the SH row
+// is handled rotated by N/2 in real space (its spectrum is then modulated by (-1)^k, which commutes with
+// every linear operation of the step): the lane that holds FH elements e, e + N/2 in registers q, q + R/2
+// has an SH partner lane that holds e + N/2, e in the same registers, so each side integrates "own lower
+// half, partner's upper half".  DESIGN.md §5.3.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -28,48 +41,79 @@ template <> struct FftCfg<1024> { static constexpr int R = 32, M = 32; };
 
 template <int N> struct Geo {
     static constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M;
-    static constexpr int G = 32 / M;                     // lines per warp
-    static constexpr int NP = N + (M == 8 ? 8 : 0);      // padded line pitch in shared memory (float2)
-    static constexpr int LINE_BYTES = NP * 8;
-    static constexpr int WARP_SMEM = 2 * G * LINE_BYTES; // scratch + park
-    static constexpr int WARPS = (N >= 512) ? 12 : 16;
+    static constexpr int G = 32 / M;                       // lines per warp
+    static constexpr int Q = R / M;                        // radix-M transforms per lane in stage B
+    static constexpr int NP = N + (M == 8 ? 8 : 0);        // line pitch in shared memory (float2)
+    static constexpr int WARP_SMEM = G * NP * 8;           // one warp's lines
+    static constexpr int WARPS = (R == 32) ? 16 : 24;
     static constexpr int THREADS = WARPS * 32;
-    static constexpr int CTA_SMEM = WARPS * WARP_SMEM;
-    // column pass: columns per warp unit (staged two at a time when a warp holds a single line)
-    static constexpr int CW = (G >= 2) ? G : 2;
+    // row pass: one item = HG rows x both fields (one warp), or one row handled by a warp pair (G == 1)
+    static constexpr int HG = (G >= 2) ? G / 2 : 1;
+    static constexpr int ROW_SLOTS = (G >= 2) ? WARPS : WARPS / 2;
+    // column pass: a team of TW warps stages a strip of SC adjacent columns (64 B per row) in shared memory
+    static constexpr int SC = 8, SCP = SC + 1;             // strip columns, padded pitch (conflict free)
+    static constexpr int TW = SC / G;                      // warps per team
+    static constexpr int TEAMS = WARPS / TW;
+    static constexpr int STRIP_SMEM = N * SCP * 8;
+    static constexpr int ROW_SMEM = WARPS * WARP_SMEM, COL_SMEM = TEAMS * STRIP_SMEM;
+    static constexpr int WORK_SMEM = ROW_SMEM > COL_SMEM ? ROW_SMEM : COL_SMEM;
+    static constexpr int TW_SMEM = N * 16;                 // twiddles [R][M] as float4 (hi.re, hi.im, lo.re, lo.im)
+    static constexpr int CTA_SMEM = WORK_SMEM + TW_SMEM;
+    static_assert(WARPS % TW == 0 && WARPS % 2 == 0, "team / pair layout");
+    static_assert(TEAMS + 1 <= 16 && WARPS / 2 + 1 <= 16, "named barrier ids");
 };
 
 __device__ __forceinline__ float2 ldcg2(const float2* p) { return __ldcg(p); }
 __device__ __forceinline__ void stcg2(float2* p, float2 v) { __stcg(p, v); }
 
+__device__ __forceinline__ void named_barrier(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
-// One line transform per M-lane group; v in/out in strided layout (thread m holds m + M q).
-// scr: this group's shared-memory line (NP float2).  tw: inter-stage twiddles W_N^e, e < N.
+// Forward transform of one line per M-lane group; v in/out in strided layout (lane m holds m + M q).
+// scr: this group's line in shared memory, slot s at scr[s * STRIDE].  tws: twiddles W_N^{k1 m} at
+// [k1 * M + m] (lanes read consecutive entries: conflict free).
 // ------------------------------------------------------------------------------------------------
-template <int N, bool INV, bool PREC>
+template <int N, int STRIDE, bool PREC>
 __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __restrict__ scr,
-                                         const float4* __restrict__ tw, int m) {
+                                         const float4* __restrict__ tws, int m) {
     constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M, Q = R / M;
-    fft_reg<R, INV, PREC>(v);
+    if constexpr (Q == 1) {
+        // both stages are the same radix: one copy of the butterfly code, executed twice
+#pragma unroll 1
+        for (int s = 0; s < 2; ++s) {
+            fft_reg<R, false, PREC>(v);
+            if (s == 0) {
 #pragma unroll
-    for (int k1 = 1; k1 < R; ++k1) {
-        float4 w = tw[k1 * m];
-        v[k1] = cmul_hl<INV, PREC>(v[k1], w);
+                for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
+#pragma unroll
+                for (int k1 = 0; k1 < R; ++k1) scr[(k1 * M + (m ^ (k1 & (M - 1)))) * STRIDE] = v[k1];
+                __syncwarp();
+#pragma unroll
+                for (int n2 = 0; n2 < M; ++n2) v[n2] = scr[(m * M + (n2 ^ m)) * STRIDE];
+                __syncwarp();
+            }
+        }
+    } else {
+        fft_reg<R, false, PREC>(v);
+#pragma unroll
+        for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
+#pragma unroll
+        for (int k1 = 0; k1 < R; ++k1) scr[(k1 * M + (m ^ (k1 & (M - 1)))) * STRIDE] = v[k1];
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            float2 u[M];
+            const int k1 = m + M * i;
+#pragma unroll
+            for (int n2 = 0; n2 < M; ++n2) u[n2] = scr[(k1 * M + (n2 ^ m)) * STRIDE];
+            fft_reg<M, false, PREC>(u);
+#pragma unroll
+            for (int k2 = 0; k2 < M; ++k2) v[i + Q * k2] = u[k2];
+        }
+        __syncwarp();
     }
-#pragma unroll
-    for (int k1 = 0; k1 < R; ++k1) scr[k1 * M + (m ^ (k1 & (M - 1)))] = v[k1];
-    __syncwarp();
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
-        float2 u[M];
-        const int k1 = m + M * i;
-#pragma unroll
-        for (int n2 = 0; n2 < M; ++n2) u[n2] = scr[k1 * M + (n2 ^ m)];
-        fft_reg<M, INV, PREC>(u);
-#pragma unroll
-        for (int k2 = 0; k2 < M; ++k2) v[i + Q * k2] = u[k2];
-    }
-    __syncwarp();
 }
 
 __device__ __forceinline__ float warp_sum(float x) {
@@ -99,8 +143,8 @@ __device__ __forceinline__ PhaseCoef phase_coef(float c, float s, float k1, floa
     return pc;
 }
 
-// dz * N(A) of P:72-73 (Eq. 2) / P:138-145 (Eq. 11) for one point.
-template <bool TPA>
+// dz * N(A) of P:72-73 (Eq. 2) / P:138-145 (Eq. 11) for one point (two-photon terms always evaluated;
+// g1 = g2 = 0 switches them off).
 __device__ __forceinline__ void nl_rhs(float2 a1, float2 a2, const PhaseCoef& pc, float g1, float g2,
                                        float2& d1, float2& d2) {
     float px = fmaf(a2.x, a1.x, a2.y * a1.y);            // A2 conj(A1)
@@ -111,26 +155,23 @@ __device__ __forceinline__ void nl_rhs(float2 a1, float2 a2, const PhaseCoef& pc
     d1.y = fmaf(px, pc.u1y, py * pc.u1x);
     d2.x = fmaf(qx, pc.u2x, -qy * pc.u2y);
     d2.y = fmaf(qx, pc.u2y, qy * pc.u2x);
-    if constexpr (TPA) {
-        float t1 = -g1 * fmaf(a1.x, a1.x, a1.y * a1.y);
-        float t2 = -g2 * fmaf(a2.x, a2.x, a2.y * a2.y);
-        d1.x = fmaf(t1, a1.x, d1.x); d1.y = fmaf(t1, a1.y, d1.y);
-        d2.x = fmaf(t2, a2.x, d2.x); d2.y = fmaf(t2, a2.y, d2.y);
-    }
+    float t1 = -g1 * fmaf(a1.x, a1.x, a1.y * a1.y);
+    float t2 = -g2 * fmaf(a2.x, a2.x, a2.y * a2.y);
+    d1.x = fmaf(t1, a1.x, d1.x); d1.y = fmaf(t1, a1.y, d1.y);
+    d2.x = fmaf(t2, a2.x, d2.x); d2.y = fmaf(t2, a2.y, d2.y);
 }
 
 // One classical RK4 step of length dz; the phase is sampled at z_n, z_n + dz/2, z_n + dz (G8).
-template <bool TPA>
 __device__ __forceinline__ void rk4_point(float2& a1, float2& a2, const PhaseCoef& ca, const PhaseCoef& cm,
                                           const PhaseCoef& cb, float g1, float g2) {
     float2 k1a, k1b, k2a, k2b, k3a, k3b, k4a, k4b;
-    nl_rhs<TPA>(a1, a2, ca, g1, g2, k1a, k1b);
-    nl_rhs<TPA>(make_float2(fmaf(0.5f, k1a.x, a1.x), fmaf(0.5f, k1a.y, a1.y)),
-                make_float2(fmaf(0.5f, k1b.x, a2.x), fmaf(0.5f, k1b.y, a2.y)), cm, g1, g2, k2a, k2b);
-    nl_rhs<TPA>(make_float2(fmaf(0.5f, k2a.x, a1.x), fmaf(0.5f, k2a.y, a1.y)),
-                make_float2(fmaf(0.5f, k2b.x, a2.x), fmaf(0.5f, k2b.y, a2.y)), cm, g1, g2, k3a, k3b);
-    nl_rhs<TPA>(make_float2(a1.x + k3a.x, a1.y + k3a.y), make_float2(a2.x + k3b.x, a2.y + k3b.y), cb, g1, g2,
-                k4a, k4b);
+    nl_rhs(a1, a2, ca, g1, g2, k1a, k1b);
+    nl_rhs(make_float2(fmaf(0.5f, k1a.x, a1.x), fmaf(0.5f, k1a.y, a1.y)),
+           make_float2(fmaf(0.5f, k1b.x, a2.x), fmaf(0.5f, k1b.y, a2.y)), cm, g1, g2, k2a, k2b);
+    nl_rhs(make_float2(fmaf(0.5f, k2a.x, a1.x), fmaf(0.5f, k2a.y, a1.y)),
+           make_float2(fmaf(0.5f, k2b.x, a2.x), fmaf(0.5f, k2b.y, a2.y)), cm, g1, g2, k3a, k3b);
+    nl_rhs(make_float2(a1.x + k3a.x, a1.y + k3a.y), make_float2(a2.x + k3b.x, a2.y + k3b.y), cb, g1, g2,
+           k4a, k4b);
     constexpr float S = 1.0f / 6.0f;
     a1.x += S * (k1a.x + 2.0f * (k2a.x + k3a.x) + k4a.x);
     a1.y += S * (k1a.y + 2.0f * (k2a.y + k3a.y) + k4a.y);
@@ -149,7 +190,6 @@ __device__ __forceinline__ float dT_lerp(const float* __restrict__ T0, size_t pl
     return a;
 }
 
-
 // Which T planes serve step node n: k = min(floor(n (nzt-1)/nz), nzt-2), f = frac.
 struct TNode { int k; float f; bool two; };
 __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
@@ -164,86 +204,80 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Row pass for one warp unit = G consecutive rows of one member, both fields.
-//   ROW_FIRST : A_in (real space) -> P_j(0) -> FFT_x -> * hx            -> A
-//   ROW_MID   : A -> inverse FFT_x -> [T -> dk -> phi] -> RK4 -> P_j(z_{n+1}) -> FFT_x -> * hx -> A
-//   ROW_FINAL : A -> inverse FFT_x -> A (output, real space)
-// hsel: 0 = full-step tables, 1 = half-step tables.  n = step index (ROW_MID).
+// Row pass, one item = HG rows x both fields.  Lane group g of the warp holds one line: field f, row r.
+// (G == 1: the item is one row and the two warps of a pair hold its two fields.)
+//   ROW_FIRST : A_in (real space) -> P_j(0) -> F_x -> * hx                          -> A
+//   ROW_MID   : A -> F_x -> conj -> [T -> dk -> phi] -> RK4 -> P_j(z_{n+1}) -> F_x -> * hx -> A
+//   ROW_FINAL : A -> F_x -> conj -> A (output, real space)
+// smem_cta: base of the per-warp line regions.  hsel: 0 = full-step tables, 1 = half-step tables.
 // ------------------------------------------------------------------------------------------------
 template <int NX, int MODE, bool PREC>
-__device__ __forceinline__ void row_unit(const Params& P, int unit, int n, int hsel, float2* smem_warp,
-                                         const float4* __restrict__ twx, int lane) {
+__device__ __forceinline__ void row_item(const Params& P, int item, int n, int hsel, float2* smem_cta,
+                                         const float4* __restrict__ tws, int warp, int lane) {
     using GE = Geo<NX>;
-    constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP;
+    constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
     const int g = lane / M, m = lane % M;
-    const int rows_per_member = P.ny;
-    const int row0 = unit * G;                       // global row index over [batch*ny]
-    const int b = row0 / rows_per_member;
-    const int y = row0 - b * rows_per_member + g;
-    const size_t rbase = ((size_t)b * P.ny + y) * NX;
-    float2* scr = smem_warp + g * NP;
-    float2* park = smem_warp + (G + g) * NP;
+    const int f = (G >= 2) ? g / HG : (warp & 1);
+    const int r = (G >= 2) ? g % HG : 0;
+    const int row = item * HG + r;                            // over [batch * ny]
+    const int b = (item * HG) / P.ny;
+    const int y = row - b * P.ny;
+    const size_t rbase = (size_t)row * NX;
+    float2* own = smem_cta + (size_t)warp * (G * NP) + g * NP;
+    float2* par = (G >= 2) ? smem_cta + (size_t)warp * (G * NP) + (g ^ HG) * NP
+                           : smem_cta + (size_t)(warp ^ 1) * (G * NP);
     const MemberDev& mb = P.mem[b];
+    const int rot = f ? NX / 2 : 0;                           // the SH row lives rotated by N/2 in real space
     float2 v[R];
 
     if constexpr (MODE == ROW_FIRST) {
-        float s[2] = {0.f, 0.f};
+        const float2* src = f ? P.Ain[1] : P.Ain[0];
+        if (src) {
 #pragma unroll
-        for (int f = 0; f < 2; ++f) {
-            const float2* src = P.Ain[f];
-            if (src) {
+            for (int q = 0; q < R; ++q) v[q] = src[rbase + ((M * q + m + rot) & (NX - 1))];
+        } else {
 #pragma unroll
-                for (int q = 0; q < R; ++q) v[q] = src[rbase + M * q + m];
-            } else {
-#pragma unroll
-                for (int q = 0; q < R; ++q) v[q] = make_float2(0.f, 0.f);
-            }
-#pragma unroll
-            for (int q = 0; q < R; ++q) s[f] += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
-            warp_fft<NX, false, PREC>(v, scr, twx, m);
-            const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
-#pragma unroll
-            for (int q = 0; q < R; ++q) {
-                v[q] = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
-                stcg2(P.A[f] + rbase + M * q + m, v[q]);
-            }
+            for (int q = 0; q < R; ++q) v[q] = make_float2(0.f, 0.f);
         }
-        float s0 = warp_sum(s[0]), s1 = warp_sum(s[1]);
+        float s = 0.f;
+#pragma unroll
+        for (int q = 0; q < R; ++q) s += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
+        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
+        float2* dst = (f ? P.A[1] : P.A[0]) + rbase;
+#pragma unroll
+        for (int q = 0; q < R; ++q) stcg2(dst + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
+        float s0 = warp_sum(f ? 0.f : s), s1 = warp_sum(f ? s : 0.f);
         if (lane == 0) {
             double* hst = P.hist + (size_t)b * (P.nz + 1) * 2;
-            atomicAdd(hst + 0, (double)s0 * mb.pscale_in[0]);
-            atomicAdd(hst + 1, (double)s1 * mb.pscale_in[1]);
+            if (G >= 2 || f == 0) atomicAdd(hst + 0, (double)s0 * mb.pscale_in[0]);
+            if (G >= 2 || f == 1) atomicAdd(hst + 1, (double)s1 * mb.pscale_in[1]);
         }
         return;
     }
 
     if constexpr (MODE == ROW_FINAL) {
+        float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
-        for (int f = 0; f < 2; ++f) {
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        warp_fft<NX, 1, PREC>(v, own, tws, m);
 #pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = ldcg2(P.A[f] + rbase + M * q + m);
-            warp_fft<NX, true, PREC>(v, scr, twx, m);
-#pragma unroll
-            for (int q = 0; q < R; ++q) stcg2(P.A[f] + rbase + M * q + m, v[q]);
-        }
+        for (int q = 0; q < R; ++q) stcg2(A + ((M * q + m + rot) & (NX - 1)), make_float2(v[q].x, -v[q].y));
         return;
     }
 
     if constexpr (MODE == ROW_MID) {
-        // ---- field 1: inverse FFT_x, park in shared memory
+        float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = ldcg2(P.A[0] + rbase + M * q + m);
-        warp_fft<NX, true, PREC>(v, scr, twx, m);
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2)
 #pragma unroll
-        for (int q = 0; q < R; ++q) park[M * q + m] = v[q];
-        // ---- field 2: inverse FFT_x, stays in registers
-#pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = ldcg2(P.A[1] + rbase + M * q + m);
-        warp_fft<NX, true, PREC>(v, scr, twx, m);
+        for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
+        if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
 
-        // ---- nonlinear step
+        // ---- nonlinear step on elements e = M q + m + f N/2, q < R/2: own lower half, partner's upper half
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz, g1 = mb.g1dz, g2 = mb.g2dz;
-        const bool tpa = (g1 != 0.f) || (g2 != 0.f);
         float s1 = 0.f, s2 = 0.f;
         if (P.nzt == 0) {
             // uniform temperature: phi(z) = dk z exactly; three sampled phases per step, warp-uniform
@@ -258,16 +292,18 @@ __device__ __forceinline__ void row_unit(const Params& P, int unit, int n, int h
             sincosf((float)pa, &sa, &ca);
             sincosf((float)pm, &sm, &cm);
             sincosf((float)pb, &sb, &cb);
-            const PhaseCoef A = phase_coef(ca, sa, k1dz, k2dz), Mi = phase_coef(cm, sm, k1dz, k2dz),
-                            B = phase_coef(cb, sb, k1dz, k2dz);
-#pragma unroll
-            for (int q = 0; q < R; ++q) {
-                float2 a1 = park[M * q + m], a2 = v[q];
-                if (tpa) rk4_point<true>(a1, a2, A, Mi, B, g1, g2);
-                else     rk4_point<false>(a1, a2, A, Mi, B, g1, g2);
+            const PhaseCoef CA = phase_coef(ca, sa, k1dz, k2dz), CM = phase_coef(cm, sm, k1dz, k2dz),
+                            CB = phase_coef(cb, sb, k1dz, k2dz);
+#pragma unroll 2
+            for (int q = 0; q < H; ++q) {
+                const float2 o = own[M * q + m], p = par[M * (q + H) + m];
+                float2 a1 = f ? p : o, a2 = f ? o : p;
+                a1.y = -a1.y; a2.y = -a2.y;
+                rk4_point(a1, a2, CA, CM, CB, g1, g2);
                 s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
                 s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
-                park[M * q + m] = a1; v[q] = a2;
+                own[M * q + m] = f ? a2 : a1;
+                par[M * (q + H) + m] = f ? a1 : a2;
             }
         } else {
             const size_t plane = (size_t)P.ny * NX;
@@ -276,30 +312,32 @@ __device__ __forceinline__ void row_unit(const Params& P, int unit, int n, int h
             const float* Ta = Tb + (size_t)ta.k * plane;
             const float* Tn = Tb + (size_t)tb.k * plane;
             const float hdz = 0.5f * mb.dz, e8 = 0.125f * mb.dz;
-            float* phi = P.phi + (size_t)b * plane;
-            const size_t pbase = (size_t)y * NX;
-#pragma unroll
-            for (int q = 0; q < R; ++q) {
-                const size_t idx = pbase + M * q + m;
+            float* phi = P.phi + (size_t)b * plane + (size_t)y * NX + rot + m;
+            const size_t pbase = (size_t)y * NX + rot + m;
+#pragma unroll 2
+            for (int q = 0; q < H; ++q) {
+                const size_t idx = pbase + M * q;
                 float dTa = dT_lerp(Ta, plane, idx, ta.f, ta.two, mb.Tpm_hi, mb.Tpm_lo);
                 float dTb = dT_lerp(Tn, plane, idx, tb.f, tb.two, mb.Tpm_hi, mb.Tpm_lo);
                 float dka = fmaf(mb.gT, dTa, mb.dk0), dkb = fmaf(mb.gT, dTb, mb.dk0);
-                float ph = __ldcg(phi + idx);
+                float ph = __ldcg(phi + M * q);
                 float phm = fmaf(e8, fmaf(3.0f, dka, dkb), ph);        // phi_n + dz (3 dk_n + dk_{n+1})/8
                 float phb = fmaf(hdz, dka + dkb, ph);                  // phi_n + dz (dk_n + dk_{n+1})/2
                 float ca, sa, cm, sm, cb, sb;
                 __sincosf(ph, &sa, &ca);
                 __sincosf(phm, &sm, &cm);
                 __sincosf(phb, &sb, &cb);
-                __stcg(phi + idx, wrap_2pi(phb));
-                const PhaseCoef A = phase_coef(ca, sa, k1dz, k2dz), Mi = phase_coef(cm, sm, k1dz, k2dz),
-                                B = phase_coef(cb, sb, k1dz, k2dz);
-                float2 a1 = park[M * q + m], a2 = v[q];
-                if (tpa) rk4_point<true>(a1, a2, A, Mi, B, g1, g2);
-                else     rk4_point<false>(a1, a2, A, Mi, B, g1, g2);
+                __stcg(phi + M * q, wrap_2pi(phb));
+                const PhaseCoef CA = phase_coef(ca, sa, k1dz, k2dz), CM = phase_coef(cm, sm, k1dz, k2dz),
+                                CB = phase_coef(cb, sb, k1dz, k2dz);
+                const float2 o = own[M * q + m], p = par[M * (q + H) + m];
+                float2 a1 = f ? p : o, a2 = f ? o : p;
+                a1.y = -a1.y; a2.y = -a2.y;
+                rk4_point(a1, a2, CA, CM, CB, g1, g2);
                 s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
                 s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
-                park[M * q + m] = a1; v[q] = a2;
+                own[M * q + m] = f ? a2 : a1;
+                par[M * (q + H) + m] = f ? a1 : a2;
             }
         }
         s1 = warp_sum(s1); s2 = warp_sum(s2);
@@ -308,103 +346,118 @@ __device__ __forceinline__ void row_unit(const Params& P, int unit, int n, int h
             atomicAdd(hst + 0, (double)s1 * mb.pscale_step[0]);
             atomicAdd(hst + 1, (double)s2 * mb.pscale_step[1]);
         }
-        // ---- field 2 forward FFT_x, propagator, store
-        {
-            warp_fft<NX, false, PREC>(v, scr, twx, m);
-            const float4* h = P.hx[hsel] + ((size_t)b * 2 + 1) * NX;
+        if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
 #pragma unroll
-            for (int q = 0; q < R; ++q)
-                stcg2(P.A[1] + rbase + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
-        }
-        // ---- field 1
-        {
+        for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
+        __syncwarp();
+        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = park[M * q + m];
-            warp_fft<NX, false, PREC>(v, scr, twx, m);
-            const float4* h = P.hx[hsel] + ((size_t)b * 2 + 0) * NX;
-#pragma unroll
-            for (int q = 0; q < R; ++q)
-                stcg2(P.A[0] + rbase + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
-        }
+        for (int q = 0; q < R; ++q) stcg2(A + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// Column pass for one warp unit = CW adjacent columns of one field of one member:
-//   FFT_y -> * hy (includes 1/(nx ny)) -> inverse FFT_y, in place.
+// Column pass, one item = a strip of SC adjacent columns of one field of one member, handled by a team of
+// TW warps:  stage the strip in shared memory (64 B per row, coalesced) -> F_y -> * hy (includes 1/(nx ny)),
+// conjugated -> F_y -> stage out.  The transposes of the two transforms run in place inside the strip.
 // ------------------------------------------------------------------------------------------------
 template <int NY, bool PREC>
-__device__ __forceinline__ void col_unit(const Params& P, int unit, int hsel, float2* smem_warp,
-                                         const float4* __restrict__ twy, int lane) {
+__device__ __forceinline__ void col_item(const Params& P, int item, int hsel, float2* strip,
+                                         const float4* __restrict__ tws, int trank, int bar_id, int lane) {
     using GE = Geo<NY>;
-    constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, CW = GE::CW;
+    constexpr int R = GE::R, M = GE::M, G = GE::G, SC = GE::SC, SCP = GE::SCP, TT = GE::TW * 32;
     const int nx = P.nx;
-    const int units_per_field = nx / CW;
-    const int bf = unit / units_per_field;           // b*2 + f
-    const int c0 = (unit - bf * units_per_field) * CW;
-    const int b = bf >> 1, f = bf & 1;
-    float2* A = P.A[f] + (size_t)b * NY * nx;
+    const int strips_per_field = nx / SC;
+    const int bf = item / strips_per_field;                   // b*2 + f
+    const int c0 = (item - bf * strips_per_field) * SC;
+    float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + c0;
     const float4* h = P.hy[hsel] + (size_t)bf * NY;
+    const int t = trank * 32 + lane;
     float2 v[R];
 
-    if constexpr (G >= 2) {
-        const int g = lane / M, m = lane % M;
-        float2* scr = smem_warp + g * NP;
-        float2* col = A + c0 + g;
+    // stage in: element i*TT + t of the strip = (row, column) = (.. / SC, .. % SC)
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = ldcg2(col + (size_t)(M * q + m) * nx);
-        warp_fft<NY, false, PREC>(v, scr, twy, m);
+    for (int i = 0; i < R; ++i) {
+        const int e = i * TT + t;
+        v[i] = ldcg2(A + (size_t)(e / SC) * nx + (e % SC));
+    }
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
-        warp_fft<NY, true, PREC>(v, scr, twy, m);
+    for (int i = 0; i < R; ++i) {
+        const int e = i * TT + t;
+        strip[(e / SC) * SCP + (e % SC)] = v[i];
+    }
+    named_barrier(bar_id, TT);
+
+    const int g = lane / M, m = lane % M;
+    float2* col = strip + trank * G + g;
 #pragma unroll
-        for (int q = 0; q < R; ++q) stcg2(col + (size_t)(M * q + m) * nx, v[q]);
-    } else {
-        // one line per warp (NY = 1024): stage two adjacent columns (16 B per row) through shared memory
-        static_assert(G >= 2 || CW == 2, "staged path handles two columns");
-        const int m = lane;
-        float2* c_a = smem_warp;             // column c0   [NY]
-        float2* c_b = smem_warp + NP;        // column c0+1 [NY]
-        const float4* src = reinterpret_cast<const float4*>(A + c0);
-        const size_t pitch4 = (size_t)nx / 2;    // row pitch in float4
+    for (int q = 0; q < R; ++q) v[q] = col[(M * q + m) * SCP];
+    __syncwarp();
+    warp_fft<NY, SCP, PREC>(v, col, tws, m);
 #pragma unroll
-        for (int q0 = 0; q0 < R; q0 += 8) {
-            float4 t[8];
+    for (int q = 0; q < R; ++q) {
+        float2 w = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
+        v[q] = make_float2(w.x, -w.y);
+    }
+    warp_fft<NY, SCP, PREC>(v, col, tws, m);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) t[j] = __ldcg(src + (size_t)(M * (q0 + j) + m) * pitch4);
+    for (int q = 0; q < R; ++q) col[(M * q + m) * SCP] = v[q];
+    named_barrier(bar_id, TT);
+
+    // stage out (each thread reads back exactly the elements it will overwrite at the next stage-in)
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                c_a[M * (q0 + j) + m] = make_float2(t[j].x, t[j].y);
-                c_b[M * (q0 + j) + m] = make_float2(t[j].z, t[j].w);
-            }
-        }
-        __syncwarp();
-#pragma unroll 1
-        for (int c = 0; c < 2; ++c) {
-            float2* cc = c ? c_b : c_a;
+    for (int i = 0; i < R; ++i) {
+        const int e = i * TT + t;
+        v[i] = strip[(e / SC) * SCP + (e % SC)];
+    }
 #pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = cc[M * q + m];
-            __syncwarp();
-            warp_fft<NY, false, PREC>(v, cc, twy, m);
-#pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
-            warp_fft<NY, true, PREC>(v, cc, twy, m);
-#pragma unroll
-            for (int q = 0; q < R; ++q) cc[M * q + m] = v[q];
-        }
-        __syncwarp();
-        float4* dst = reinterpret_cast<float4*>(A + c0);
-#pragma unroll
-        for (int q = 0; q < R; ++q) {
-            float2 a = c_a[M * q + m], bb = c_b[M * q + m];
-            __stcg(dst + (size_t)(M * q + m) * pitch4, make_float4(a.x, a.y, bb.x, bb.y));
-        }
-        __syncwarp();
+    for (int i = 0; i < R; ++i) {
+        const int e = i * TT + t;
+        stcg2(A + (size_t)(e / SC) * nx + (e % SC), v[i]);
     }
 }
 
-template <int NX> __host__ __device__ inline int row_units(int batch, int ny) { return batch * ny / Geo<NX>::G; }
-template <int NY> __host__ __device__ inline int col_units(int batch, int nx) { return batch * 2 * nx / Geo<NY>::CW; }
+template <int NX> __host__ __device__ inline int row_items(int batch, int ny) { return batch * ny / Geo<NX>::HG; }
+template <int NY> __host__ __device__ inline int col_items(int batch, int nx) { return batch * 2 * (nx / Geo<NY>::SC); }
+
+// Balanced static schedule: CTA c owns items [U c / grid, U (c+1) / grid); inside the CTA they go round
+// robin to the slots (warps, warp pairs or teams), so the four schedulers of an SM differ by <= 1 item.
+__device__ __forceinline__ void cta_range(int U, int& lo, int& hi) {
+    lo = (int)(((long long)U * blockIdx.x) / gridDim.x);
+    hi = (int)(((long long)U * (blockIdx.x + 1)) / gridDim.x);
+}
+
+template <int N>
+__device__ __forceinline__ const float4* load_twiddles(unsigned char* smem_raw, const float4* __restrict__ tw) {
+    float4* tws = reinterpret_cast<float4*>(smem_raw + Geo<N>::WORK_SMEM);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) tws[i] = tw[i];
+    __syncthreads();
+    return tws;
+}
+
+template <int NX, int MODE, bool PREC>
+__device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float2* smem_cta,
+                                         const float4* __restrict__ tws, int warp, int lane) {
+    using GE = Geo<NX>;
+    int lo, hi;
+    cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
+    const int slot = (GE::G >= 2) ? warp : (warp >> 1);
+    for (int it = lo + slot; it < hi; it += GE::ROW_SLOTS)
+        row_item<NX, MODE, PREC>(P, it, n, hsel, smem_cta, tws, warp, lane);
+}
+
+template <int NY, bool PREC>
+__device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem_cta,
+                                         const float4* __restrict__ tws, int warp, int lane) {
+    using GE = Geo<NY>;
+    int lo, hi;
+    cta_range(col_items<NY>(P.batch, P.nx), lo, hi);
+    const int team = warp / GE::TW, trank = warp % GE::TW;
+    float2* strip = smem_cta + (size_t)team * (NY * GE::SCP);
+    for (int it = lo + team; it < hi; it += GE::TEAMS)
+        col_item<NY, PREC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
+}
 
 // ------------------------------------------------------------------------------------------------
 // Per-pass kernels (two launches per z-step; any nx, ny)
@@ -413,20 +466,16 @@ template <int NX, int MODE, bool PREC>
 __global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row(Params P, int n, int hsel) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* smem_warp = reinterpret_cast<float2*>(smem_raw + (size_t)warp * Geo<NX>::WARP_SMEM);
-    const int U = row_units<NX>(P.batch, P.ny);
-    for (int u = blockIdx.x + gridDim.x * warp; u < U; u += gridDim.x * Geo<NX>::WARPS)
-        row_unit<NX, MODE, PREC>(P, u, n, hsel, smem_warp, P.twx, lane);
+    const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
+    row_pass<NX, MODE, PREC>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 template <int NY, bool PREC>
 __global__ void __launch_bounds__(Geo<NY>::THREADS, 1) k_col(Params P, int hsel) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* smem_warp = reinterpret_cast<float2*>(smem_raw + (size_t)warp * Geo<NY>::WARP_SMEM);
-    const int U = col_units<NY>(P.batch, P.nx);
-    for (int u = blockIdx.x + gridDim.x * warp; u < U; u += gridDim.x * Geo<NY>::WARPS)
-        col_unit<NY, PREC>(P, u, hsel, smem_warp, P.twy, lane);
+    const float4* tws = load_twiddles<NY>(smem_raw, P.twy);
+    col_pass<NY, PREC>(P, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -467,19 +516,15 @@ template <int N, bool PREC>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* smem_warp = reinterpret_cast<float2*>(smem_raw + (size_t)warp * Geo<N>::WARP_SMEM);
-    float4* tw_s = reinterpret_cast<float4*>(smem_raw + Geo<N>::CTA_SMEM);   // [N] twiddles (twx == twy)
-    for (int i = threadIdx.x; i < N; i += blockDim.x) tw_s[i] = P.twx[i];
-    __syncthreads();
-    const int UR = row_units<N>(P.batch, P.ny), UC = col_units<N>(P.batch, P.nx);
+    const float4* tws = load_twiddles<N>(smem_raw, P.twx);   // twx == twy on a square grid
+    float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
     unsigned int epoch = 0;
+#pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        for (int u = blockIdx.x + gridDim.x * warp; u < UR; u += gridDim.x * Geo<N>::WARPS)
-            row_unit<N, ROW_MID, PREC>(P, u, n, hsel, smem_warp, tw_s, lane);
+        row_pass<N, ROW_MID, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch)) return;
-        for (int u = blockIdx.x + gridDim.x * warp; u < UC; u += gridDim.x * Geo<N>::WARPS)
-            col_unit<N, PREC>(P, u, hsel, smem_warp, tw_s, lane);
+        col_pass<N, PREC>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch)) return;
     }
 }

@@ -36,7 +36,7 @@ cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
 
 template <bool PREC>
 cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
-    const int smem = GE::CTA_SMEM + N * (int)sizeof(float4);
+    const int smem = GE::CTA_SMEM;
     cudaError_t e = set_smem(k_persist<N, PREC>, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -76,9 +76,11 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
 
 LaunchInfo SHG_CAT(launch_info_, SHG_N)() {
     LaunchInfo li;
-    li.lines_per_warp = GE::G;
-    li.cols_per_unit = GE::CW;
+    li.rows_per_item = GE::HG;
+    li.cols_per_item = GE::SC;
     li.warps = GE::WARPS;
+    li.fft_r = GE::R;
+    li.fft_m = GE::M;
     return li;
 }
 

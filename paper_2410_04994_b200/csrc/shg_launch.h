@@ -8,9 +8,10 @@ namespace shg {
 struct Params;
 
 struct LaunchInfo {
-    int lines_per_warp;   // G: rows per row-pass warp unit
-    int cols_per_unit;    // CW: columns per column-pass warp unit
+    int rows_per_item;    // HG: rows (both fields) per row-pass item
+    int cols_per_item;    // SC: columns per column-pass strip
     int warps;            // warps per CTA
+    int fft_r, fft_m;     // line length = fft_r * fft_m; twiddle table layout [fft_r][fft_m]
 };
 
 #define SHG_DECLARE_N(N)                                                                                   \
