@@ -394,6 +394,26 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const int UC = batch * 2 * (g.nx / iy.cols_per_item);    // column-pass strips
     const int grid_r = UR < ctx->sm_count ? UR : ctx->sm_count;
     const int grid_c = UC < ctx->sm_count ? UC : ctx->sm_count;
+    const bool use_persist = ctx->persistent && g.nx == g.ny;
+    // How many slots / teams of a CTA take items.  A CTA owns ipc = ceil(U / grid) items; they are dealt round
+    // robin, so with `rounds` = ceil(ipc / slots) rounds it is better to use just enough slots for full
+    // rounds (every busy warp then runs the same number of items back to back) than to leave a ragged last
+    // round in which a few warps run alone.  Rounded up so that the busy warps spread evenly over the four
+    // schedulers of the SM.
+    auto active = [](int U, int grid, int slots, int warps_per_slot) {
+        const int ipc = (U + grid - 1) / grid;
+        const int rounds = (ipc + slots - 1) / slots;
+        int act = (ipc + rounds - 1) / rounds;
+        const int mult = warps_per_slot >= 4 ? 1 : 4 / warps_per_slot;
+        act = (act + mult - 1) / mult * mult;
+        return act < slots ? act : slots;
+    };
+    {
+        const int gr = use_persist ? (grid_r > grid_c ? grid_r : grid_c) : grid_r;
+        const int gc = use_persist ? gr : grid_c;
+        P.row_slots = active(UR, gr, ix.row_slots, ix.warps / ix.row_slots);
+        P.col_teams = active(UC, gc, iy.col_teams, iy.team_warps);
+    }
     const bool prec = ctx->precise;
     int launches = 0;
 
@@ -401,7 +421,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 1, prec, grid_r, st)); ++launches;
     CU(ctx->Ly.col(P, 1, prec, grid_c, st)); ++launches;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
-    if (ctx->persistent && g.nx == g.ny) {
+    if (use_persist) {
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
         CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
     } else {

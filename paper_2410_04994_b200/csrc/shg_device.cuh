@@ -43,18 +43,25 @@ template <int N> struct Geo {
     static constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M;
     static constexpr int G = 32 / M;                       // lines per warp
     static constexpr int Q = R / M;                        // radix-M transforms per lane in stage B
-    static constexpr int NP = N + (M == 8 ? 8 : 0);        // line pitch in shared memory (float2)
+    static constexpr int MP = M + 1;                       // padded pitch of the in-line transpose
+    static constexpr int LP = R * MP;                      // float2 slots one line needs (>= N)
+    // line pitch in shared memory (float2): with M = 8 two lines share a 16-lane wavefront and must start
+    // 16 banks apart (pitch = 8 mod 16)
+    static constexpr int NP = (M == 8) ? ((LP + 7) / 16 * 16 + 8) : LP;
     static constexpr int WARP_SMEM = G * NP * 8;           // one warp's lines
-    static constexpr int WARPS = (R == 32) ? 16 : 24;
+    static constexpr int WARPS = 16;
     static constexpr int THREADS = WARPS * 32;
     // row pass: one item = HG rows x both fields (one warp), or one row handled by a warp pair (G == 1)
     static constexpr int HG = (G >= 2) ? G / 2 : 1;
     static constexpr int ROW_SLOTS = (G >= 2) ? WARPS : WARPS / 2;
     // column pass: a team of TW warps stages a strip of SC adjacent columns (64 B per row) in shared memory
-    static constexpr int SC = 8, SCP = SC + 1;             // strip columns, padded pitch (conflict free)
+    // The strip is stored column by column, one line of pitch CP per column; CP = 2 mod 16 makes the
+    // staging stores (8 columns x 2 rows per 16-lane wavefront) conflict free.
+    static constexpr int SC = 8;                           // strip columns
+    static constexpr int CP = (LP + 13) / 16 * 16 + 2;     // column line pitch (float2), >= LP
     static constexpr int TW = SC / G;                      // warps per team
     static constexpr int TEAMS = WARPS / TW;
-    static constexpr int STRIP_SMEM = N * SCP * 8;
+    static constexpr int STRIP_SMEM = SC * CP * 8;
     static constexpr int ROW_SMEM = WARPS * WARP_SMEM, COL_SMEM = TEAMS * STRIP_SMEM;
     static constexpr int WORK_SMEM = ROW_SMEM > COL_SMEM ? ROW_SMEM : COL_SMEM;
     static constexpr int TW_SMEM = N * 16;                 // twiddles [R][M] as float4 (hi.re, hi.im, lo.re, lo.im)
@@ -72,13 +79,16 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads) {
 
 // ------------------------------------------------------------------------------------------------
 // Forward transform of one line per M-lane group; v in/out in strided layout (lane m holds m + M q).
-// scr: this group's line in shared memory, slot s at scr[s * STRIDE].  tws: twiddles W_N^{k1 m} at
-// [k1 * M + m] (lanes read consecutive entries: conflict free).
+// line: this group's line in shared memory (Geo<N>::LP slots; the transpose is padded, so every address is
+// a per-lane base plus a compile-time offset and every access is conflict free).  tws: twiddles
+// W_N^{k1 m} at [k1 * M + m] (lanes read consecutive entries).
 // ------------------------------------------------------------------------------------------------
-template <int N, int STRIDE, bool PREC>
-__device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __restrict__ scr,
+template <int N, bool PREC>
+__device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __restrict__ line,
                                          const float4* __restrict__ tws, int m) {
-    constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M, Q = R / M;
+    constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M, Q = R / M, MP = M + 1;
+    float2* wr = line + m;            // transpose: value (k1, lane m) goes to slot k1 * MP + m ...
+    float2* rd = line + m * MP;       // ... and lane m collects row k1 = m (+ M i): slots k1 * MP + n2
     if constexpr (Q == 1) {
         // both stages are the same radix: one copy of the butterfly code, executed twice
 #pragma unroll 1
@@ -88,10 +98,10 @@ __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __re
 #pragma unroll
                 for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
 #pragma unroll
-                for (int k1 = 0; k1 < R; ++k1) scr[(k1 * M + (m ^ (k1 & (M - 1)))) * STRIDE] = v[k1];
+                for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
                 __syncwarp();
 #pragma unroll
-                for (int n2 = 0; n2 < M; ++n2) v[n2] = scr[(m * M + (n2 ^ m)) * STRIDE];
+                for (int n2 = 0; n2 < M; ++n2) v[n2] = rd[n2];
                 __syncwarp();
             }
         }
@@ -100,14 +110,13 @@ __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __re
 #pragma unroll
         for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
 #pragma unroll
-        for (int k1 = 0; k1 < R; ++k1) scr[(k1 * M + (m ^ (k1 & (M - 1)))) * STRIDE] = v[k1];
+        for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
         __syncwarp();
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             float2 u[M];
-            const int k1 = m + M * i;
 #pragma unroll
-            for (int n2 = 0; n2 < M; ++n2) u[n2] = scr[(k1 * M + (n2 ^ m)) * STRIDE];
+            for (int n2 = 0; n2 < M; ++n2) u[n2] = rd[i * M * MP + n2];
             fft_reg<M, false, PREC>(u);
 #pragma unroll
             for (int k2 = 0; k2 < M; ++k2) v[i + Q * k2] = u[k2];
@@ -242,7 +251,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float s = 0.f;
 #pragma unroll
         for (int q = 0; q < R; ++q) s += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
-        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        warp_fft<NX, PREC>(v, own, tws, m);
         const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
         float2* dst = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
@@ -260,7 +269,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
-        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        warp_fft<NX, PREC>(v, own, tws, m);
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + ((M * q + m + rot) & (NX - 1)), make_float2(v[q].x, -v[q].y));
         return;
@@ -270,7 +279,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
-        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        warp_fft<NX, PREC>(v, own, tws, m);
         // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2)
 #pragma unroll
         for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
@@ -350,7 +359,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
         __syncwarp();
-        warp_fft<NX, 1, PREC>(v, own, tws, m);
+        warp_fft<NX, PREC>(v, own, tws, m);
         const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
@@ -360,62 +369,56 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 // ------------------------------------------------------------------------------------------------
 // Column pass, one item = a strip of SC adjacent columns of one field of one member, handled by a team of
 // TW warps:  stage the strip in shared memory (64 B per row, coalesced) -> F_y -> * hy (includes 1/(nx ny)),
-// conjugated -> F_y -> stage out.  The transposes of the two transforms run in place inside the strip.
+// conjugated -> F_y -> stage out.  The strip is held column by column, so each column is a line the
+// transform can transpose in place.
 // ------------------------------------------------------------------------------------------------
 template <int NY, bool PREC>
 __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, float2* strip,
                                          const float4* __restrict__ tws, int trank, int bar_id, int lane) {
     using GE = Geo<NY>;
-    constexpr int R = GE::R, M = GE::M, G = GE::G, SC = GE::SC, SCP = GE::SCP, TT = GE::TW * 32;
+    constexpr int R = GE::R, M = GE::M, G = GE::G, SC = GE::SC, CP = GE::CP, TT = GE::TW * 32;
     const int nx = P.nx;
     const int strips_per_field = nx / SC;
     const int bf = item / strips_per_field;                   // b*2 + f
     const int c0 = (item - bf * strips_per_field) * SC;
-    float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + c0;
-    const float4* h = P.hy[hsel] + (size_t)bf * NY;
     const int t = trank * 32 + lane;
+    // staging: thread t moves elements (row, column) = (t / SC + i TT / SC, t % SC), i = 0..R-1
+    float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + c0 + (size_t)(t / SC) * nx + (t % SC);
+    const size_t gstep = (size_t)(TT / SC) * nx;
+    float2* st = strip + (t % SC) * CP + (t / SC);
+    const float4* h = P.hy[hsel] + (size_t)bf * NY;
     float2 v[R];
 
-    // stage in: element i*TT + t of the strip = (row, column) = (.. / SC, .. % SC)
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int e = i * TT + t;
-        v[i] = ldcg2(A + (size_t)(e / SC) * nx + (e % SC));
-    }
+    for (int i = 0; i < R; ++i) v[i] = ldcg2(A + i * gstep);
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int e = i * TT + t;
-        strip[(e / SC) * SCP + (e % SC)] = v[i];
-    }
+    for (int i = 0; i < R; ++i) st[i * (TT / SC)] = v[i];
     named_barrier(bar_id, TT);
 
+    // lane group g of warp trank owns one column; with four groups per warp the two groups that share a
+    // wavefront take columns 4 apart (their lines then start 16 banks apart)
     const int g = lane / M, m = lane % M;
-    float2* col = strip + trank * G + g;
+    const int cg = (G == 4) ? (trank * 2 + (g >> 1) + 4 * (g & 1)) : (trank * G + g);
+    float2* line = strip + cg * CP;
 #pragma unroll
-    for (int q = 0; q < R; ++q) v[q] = col[(M * q + m) * SCP];
+    for (int q = 0; q < R; ++q) v[q] = line[M * q + m];
     __syncwarp();
-    warp_fft<NY, SCP, PREC>(v, col, tws, m);
+    warp_fft<NY, PREC>(v, line, tws, m);
 #pragma unroll
     for (int q = 0; q < R; ++q) {
         float2 w = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
         v[q] = make_float2(w.x, -w.y);
     }
-    warp_fft<NY, SCP, PREC>(v, col, tws, m);
+    warp_fft<NY, PREC>(v, line, tws, m);
 #pragma unroll
-    for (int q = 0; q < R; ++q) col[(M * q + m) * SCP] = v[q];
+    for (int q = 0; q < R; ++q) line[M * q + m] = v[q];
     named_barrier(bar_id, TT);
 
     // stage out (each thread reads back exactly the elements it will overwrite at the next stage-in)
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int e = i * TT + t;
-        v[i] = strip[(e / SC) * SCP + (e % SC)];
-    }
+    for (int i = 0; i < R; ++i) v[i] = st[i * (TT / SC)];
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const int e = i * TT + t;
-        stcg2(A + (size_t)(e / SC) * nx + (e % SC), v[i]);
-    }
+    for (int i = 0; i < R; ++i) stcg2(A + i * gstep, v[i]);
 }
 
 template <int NX> __host__ __device__ inline int row_items(int batch, int ny) { return batch * ny / Geo<NX>::HG; }
@@ -443,7 +446,8 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
     int lo, hi;
     cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
-    for (int it = lo + slot; it < hi; it += GE::ROW_SLOTS)
+    if (slot >= P.row_slots) return;
+    for (int it = lo + slot; it < hi; it += P.row_slots)
         row_item<NX, MODE, PREC>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
 
@@ -454,8 +458,9 @@ __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem
     int lo, hi;
     cta_range(col_items<NY>(P.batch, P.nx), lo, hi);
     const int team = warp / GE::TW, trank = warp % GE::TW;
-    float2* strip = smem_cta + (size_t)team * (NY * GE::SCP);
-    for (int it = lo + team; it < hi; it += GE::TEAMS)
+    float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
+    if (team >= P.col_teams) return;
+    for (int it = lo + team; it < hi; it += P.col_teams)
         col_item<NY, PREC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
 }
 

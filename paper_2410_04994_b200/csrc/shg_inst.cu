@@ -79,6 +79,9 @@ LaunchInfo SHG_CAT(launch_info_, SHG_N)() {
     li.rows_per_item = GE::HG;
     li.cols_per_item = GE::SC;
     li.warps = GE::WARPS;
+    li.row_slots = GE::ROW_SLOTS;
+    li.col_teams = GE::TEAMS;
+    li.team_warps = GE::TW;
     li.fft_r = GE::R;
     li.fft_m = GE::M;
     return li;

@@ -11,6 +11,9 @@ struct LaunchInfo {
     int rows_per_item;    // HG: rows (both fields) per row-pass item
     int cols_per_item;    // SC: columns per column-pass strip
     int warps;            // warps per CTA
+    int row_slots;        // slots per CTA that can take row items (warps, or warp pairs at N = 1024)
+    int col_teams;        // teams per CTA that can take strips
+    int team_warps;       // warps per team
     int fft_r, fft_m;     // line length = fft_r * fft_m; twiddle table layout [fft_r][fft_m]
 };
 
