@@ -77,6 +77,54 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// Table loads whose address carries a (numerically void) dependency on an earlier result.  Without it ptxas
+// hoists all R twiddle / propagator loads (4 registers each) far above their use and spills the line data
+// to make room; chaining load k to product k - TABLE_DEPTH keeps TABLE_DEPTH loads in flight.  One LOP3 each.
+constexpr int TABLE_DEPTH = 6;
+
+template <int BYTE_OFF>
+__device__ __forceinline__ float4 lds128_after(unsigned saddr, float dep) {
+    unsigned a;
+    asm("lop3.b32 %0, %1, %2, 0, 0xF8;" : "=r"(a) : "r"(saddr), "r"(__float_as_uint(dep)));   // a | (dep & 0)
+    float4 w;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+        : "=f"(w.x), "=f"(w.y), "=f"(w.z), "=f"(w.w) : "r"(a), "n"(BYTE_OFF));
+    return w;
+}
+
+__device__ __forceinline__ const float4* ptr_after(const float4* p, float dep) {
+    unsigned lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(p));
+    asm("lop3.b32 %0, %0, %1, 0, 0xF8;" : "+r"(lo) : "r"(__float_as_uint(dep)));
+    const float4* r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+
+// v[q] *= table[M q] for q = 0..R-1 (table already offset by the lane), loads chained TABLE_DEPTH deep
+template <int R, int M, bool PREC, bool CONJ_OUT>
+__device__ __forceinline__ void table_mul(float2 (&v)[R], const float4* __restrict__ tab) {
+#pragma unroll
+    for (int q = 0; q < R; ++q) {
+        const float dep = (q >= TABLE_DEPTH) ? v[q - TABLE_DEPTH].x : v[q].x;
+        const float2 w = cmul_hl<false, PREC>(v[q], __ldg(ptr_after(tab, dep) + M * q));
+        v[q] = CONJ_OUT ? make_float2(w.x, -w.y) : w;
+    }
+}
+
+template <int N, bool PREC, int K1>
+__device__ __forceinline__ void twiddle_one(float2 (&v)[FftCfg<N>::R], unsigned tws_saddr) {
+    constexpr int M = FftCfg<N>::M;
+    const float dep = (K1 > TABLE_DEPTH) ? v[K1 - TABLE_DEPTH].x : v[K1].x;
+    v[K1] = cmul_hl<false, PREC>(v[K1], lds128_after<K1 * M * 16>(tws_saddr, dep));
+}
+
+template <int N, bool PREC, int... K>
+__device__ __forceinline__ void twiddle_all(float2 (&v)[FftCfg<N>::R], unsigned tws_saddr,
+                                            std::integer_sequence<int, K...>) {
+    (twiddle_one<N, PREC, K + 1>(v, tws_saddr), ...);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Forward transform of one line per M-lane group; v in/out in strided layout (lane m holds m + M q).
 // line: this group's line in shared memory (Geo<N>::LP slots; the transpose is padded, so every address is
@@ -87,6 +135,7 @@ template <int N, bool PREC>
 __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __restrict__ line,
                                          const float4* __restrict__ tws, int m) {
     constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M, Q = R / M, MP = M + 1;
+    const unsigned tws_saddr = (unsigned)__cvta_generic_to_shared(tws + m);
     float2* wr = line + m;            // transpose: value (k1, lane m) goes to slot k1 * MP + m ...
     float2* rd = line + m * MP;       // ... and lane m collects row k1 = m (+ M i): slots k1 * MP + n2
     if constexpr (Q == 1) {
@@ -95,8 +144,7 @@ __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __re
         for (int s = 0; s < 2; ++s) {
             fft_reg<R, false, PREC>(v);
             if (s == 0) {
-#pragma unroll
-                for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
+                twiddle_all<N, PREC>(v, tws_saddr, std::make_integer_sequence<int, R - 1>{});
 #pragma unroll
                 for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
                 __syncwarp();
@@ -107,8 +155,7 @@ __device__ __forceinline__ void warp_fft(float2 (&v)[FftCfg<N>::R], float2* __re
         }
     } else {
         fft_reg<R, false, PREC>(v);
-#pragma unroll
-        for (int k1 = 1; k1 < R; ++k1) v[k1] = cmul_hl<false, PREC>(v[k1], tws[k1 * M + m]);
+        twiddle_all<N, PREC>(v, tws_saddr, std::make_integer_sequence<int, R - 1>{});
 #pragma unroll
         for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
         __syncwarp();
@@ -188,12 +235,26 @@ __device__ __forceinline__ void rk4_point(float2& a1, float2& a2, const PhaseCoe
     a2.y += S * (k1b.y + 2.0f * (k2b.y + k3b.y) + k4b.y);
 }
 
-// Temperature rise T - T_pm at one point of plane pair (k, k+1) with weight f  (G15).
-__device__ __forceinline__ float dT_lerp(const float* __restrict__ T0, size_t plane, size_t idx, float f,
-                                         bool two, float Thi, float Tlo) {
-    float a = (__ldg(T0 + idx) - Thi) - Tlo;
+// Raw operands of one point's phase update: the (up to) two temperature planes around z_n and around
+// z_{n+1}, and the running phase.  Loaded one RK4 iteration ahead of their use (software pipeline).
+struct TPoint { float a0, a1, b0, b1, ph; };
+
+__device__ __forceinline__ TPoint t_load(const float* __restrict__ Ta, const float* __restrict__ Tn, size_t plane,
+                                         size_t idx, bool two_a, bool two_b, const float* __restrict__ phi_q) {
+    TPoint t;
+    t.a0 = __ldg(Ta + idx);
+    t.a1 = two_a ? __ldg(Ta + plane + idx) : 0.f;
+    t.b0 = __ldg(Tn + idx);
+    t.b1 = two_b ? __ldg(Tn + plane + idx) : 0.f;
+    t.ph = __ldcg(phi_q);
+    return t;
+}
+
+// Temperature rise T - T_pm from a plane pair (k, k+1) with weight f  (G15).
+__device__ __forceinline__ float dT_lerp(float t0, float t1, float f, bool two, float Thi, float Tlo) {
+    float a = (t0 - Thi) - Tlo;
     if (two) {
-        float b = (__ldg(T0 + plane + idx) - Thi) - Tlo;
+        float b = (t1 - Thi) - Tlo;
         a = fmaf(f, b - a, a);
     }
     return a;
@@ -252,10 +313,10 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 #pragma unroll
         for (int q = 0; q < R; ++q) s += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
         warp_fft<NX, PREC>(v, own, tws, m);
-        const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
+        table_mul<R, M, PREC, false>(v, P.hx[hsel] + ((size_t)b * 2 + f) * NX + m);
         float2* dst = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
-        for (int q = 0; q < R; ++q) stcg2(dst + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
+        for (int q = 0; q < R; ++q) stcg2(dst + M * q + m, v[q]);
         float s0 = warp_sum(f ? 0.f : s), s1 = warp_sum(f ? s : 0.f);
         if (lane == 0) {
             double* hst = P.hist + (size_t)b * (P.nz + 1) * 2;
@@ -279,6 +340,21 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        // temperature / phase operands of the first RK4 point are requested before the transform
+        const size_t plane = (size_t)P.ny * NX;
+        const size_t pbase = (size_t)y * NX + rot + m;
+        const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
+        const float* Ta = nullptr;
+        const float* Tn = nullptr;
+        float* phi = nullptr;
+        TPoint cur{};
+        if (P.nzt != 0) {
+            const float* Tb = P.T + (P.T_per_member ? (size_t)b * P.nzt * plane : 0);
+            Ta = Tb + (size_t)ta.k * plane;
+            Tn = Tb + (size_t)tb.k * plane;
+            phi = P.phi + (size_t)b * plane + pbase;
+            cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
+        }
         warp_fft<NX, PREC>(v, own, tws, m);
         // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2)
 #pragma unroll
@@ -315,21 +391,15 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                 par[M * (q + H) + m] = f ? a1 : a2;
             }
         } else {
-            const size_t plane = (size_t)P.ny * NX;
-            const float* Tb = P.T + (P.T_per_member ? (size_t)b * P.nzt * plane : 0);
-            const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
-            const float* Ta = Tb + (size_t)ta.k * plane;
-            const float* Tn = Tb + (size_t)tb.k * plane;
             const float hdz = 0.5f * mb.dz, e8 = 0.125f * mb.dz;
-            float* phi = P.phi + (size_t)b * plane + (size_t)y * NX + rot + m;
-            const size_t pbase = (size_t)y * NX + rot + m;
 #pragma unroll 2
             for (int q = 0; q < H; ++q) {
-                const size_t idx = pbase + M * q;
-                float dTa = dT_lerp(Ta, plane, idx, ta.f, ta.two, mb.Tpm_hi, mb.Tpm_lo);
-                float dTb = dT_lerp(Tn, plane, idx, tb.f, tb.two, mb.Tpm_hi, mb.Tpm_lo);
+                const TPoint tp = cur;
+                if (q + 1 < H) cur = t_load(Ta, Tn, plane, pbase + M * (q + 1), ta.two, tb.two, phi + M * (q + 1));
+                float dTa = dT_lerp(tp.a0, tp.a1, ta.f, ta.two, mb.Tpm_hi, mb.Tpm_lo);
+                float dTb = dT_lerp(tp.b0, tp.b1, tb.f, tb.two, mb.Tpm_hi, mb.Tpm_lo);
                 float dka = fmaf(mb.gT, dTa, mb.dk0), dkb = fmaf(mb.gT, dTb, mb.dk0);
-                float ph = __ldcg(phi + M * q);
+                float ph = tp.ph;
                 float phm = fmaf(e8, fmaf(3.0f, dka, dkb), ph);        // phi_n + dz (3 dk_n + dk_{n+1})/8
                 float phb = fmaf(hdz, dka + dkb, ph);                  // phi_n + dz (dk_n + dk_{n+1})/2
                 float ca, sa, cm, sm, cb, sb;
@@ -360,9 +430,9 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
-        const float4* h = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
+        table_mul<R, M, PREC, false>(v, P.hx[hsel] + ((size_t)b * 2 + f) * NX + m);
 #pragma unroll
-        for (int q = 0; q < R; ++q) stcg2(A + M * q + m, cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m)));
+        for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
     }
 }
 
@@ -404,11 +474,7 @@ __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, fl
     for (int q = 0; q < R; ++q) v[q] = line[M * q + m];
     __syncwarp();
     warp_fft<NY, PREC>(v, line, tws, m);
-#pragma unroll
-    for (int q = 0; q < R; ++q) {
-        float2 w = cmul_hl<false, PREC>(v[q], __ldg(h + M * q + m));
-        v[q] = make_float2(w.x, -w.y);
-    }
+    table_mul<R, M, PREC, true>(v, h + m);
     warp_fft<NY, PREC>(v, line, tws, m);
 #pragma unroll
     for (int q = 0; q < R; ++q) line[M * q + m] = v[q];
