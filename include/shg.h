@@ -78,6 +78,12 @@ typedef struct {
                                   fp32 hi+lo pair whose lo part enters the FMA addend, so constant rounding
                                   does not accumulate linearly over thousands of z-steps; 0: plain fp32.  */
 
+#define SHG_OPT_TRACE      3   /* value = number of leading z-steps whose phase timeline the persistent kernel
+                                  records (0 = off, default; <= 4096): per step, CTA and device-wide barrier
+                                  (0 = after the row pass, 1 = after the column pass) four int64: SM clock when
+                                  the CTA finished its share of the pass, SM clock when the barrier released it,
+                                  %globaltimer (ns) at release, SM id.  Read back with shg_read_trace.            */
+
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);
 
@@ -124,6 +130,11 @@ int shg_gaussian_input(shg_ctx* ctx, void* A1_device, int batch, void* cuda_stre
  * opening / closing half-step launches are outside.  shg_last_main_loop_ms synchronises the stream. */
 int shg_enable_timing(shg_ctx* ctx, int on);
 int shg_last_main_loop_ms(shg_ctx* ctx, float* ms);
+
+/* Phase timeline of the last shg_propagate run with SHG_OPT_TRACE (persistent kernel only).
+ * out: HOST int64 [*steps][*grid][2][4] (see SHG_OPT_TRACE); out == NULL only queries *steps and *grid.
+ * Synchronises the stream of the last propagate. */
+int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid);
 
 /* Number of kernels the last shg_propagate / shg_propagate_host launched. */
 int shg_last_launch_count(const shg_ctx* ctx);

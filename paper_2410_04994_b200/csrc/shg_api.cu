@@ -103,6 +103,9 @@ struct shg_ctx {
     float* d_T_owned = nullptr;
     size_t T_owned_bytes = 0;
     float2* d_stage[2] = {nullptr, nullptr};
+    long long* d_trace = nullptr;
+    int trace_steps = 0;        // steps recorded per propagate (0 = tracing off)
+    int trace_grid = 0;         // CTAs of the last traced launch
 
     const float* d_T = nullptr;
     double T_uniform = 0.0;
@@ -241,6 +244,7 @@ void free_ctx(shg_ctx* ctx) {
     cudaFree(ctx->d_hist);
     cudaFree(ctx->d_barrier);
     cudaFree(ctx->d_T_owned);
+    cudaFree(ctx->d_trace);
     for (int i = 0; i < 2; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
@@ -325,6 +329,22 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
         case SHG_OPT_PRECISE:
             if (ctx->precise != (value != 0)) { ctx->precise = (value != 0); ctx->tables_dirty = true; }
             return SHG_OK;
+        case SHG_OPT_TRACE: {
+            if (value < 0 || value > 4096) return SHG_EINVAL;
+            if (value != ctx->trace_steps) {
+                CU(cudaStreamSynchronize(ctx->last_stream));
+                cudaFree(ctx->d_trace);
+                ctx->d_trace = nullptr;
+                ctx->trace_steps = 0;
+                if (value > 0) {
+                    const size_t bytes = sizeof(long long) * (size_t)value * ctx->sm_count * 8;
+                    CU(cudaMalloc((void**)&ctx->d_trace, bytes));
+                    CU(cudaMemset(ctx->d_trace, 0, bytes));
+                    ctx->trace_steps = value;
+                }
+            }
+            return SHG_OK;
+        }
         default: return SHG_EINVAL;
     }
 }
@@ -383,6 +403,8 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.hist = ctx->d_hist;
     P.barrier = ctx->d_barrier;
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
+    P.trace = ctx->d_trace;
+    P.trace_steps = ctx->trace_steps;
 
     const size_t np = np_of(ctx);
     CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(double) * (size_t)g.batch * (g.nz + 1) * 2, st));
@@ -423,6 +445,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
     if (use_persist) {
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
+        ctx->trace_grid = grid_p;
         CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
     } else {
         for (int n = 0; n < g.nz; ++n) {
@@ -533,6 +556,17 @@ int shg_last_main_loop_ms(shg_ctx* ctx, float* ms) {
     if (!ctx->ev_recorded) return SHG_ESTATE;
     CU(cudaEventSynchronize(ctx->ev[1]));
     CU(cudaEventElapsedTime(ms, ctx->ev[0], ctx->ev[1]));
+    return SHG_OK;
+}
+
+int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid) {
+    if (!ctx || !steps || !grid) return SHG_EINVAL;
+    *steps = ctx->trace_steps < ctx->g.nz ? ctx->trace_steps : ctx->g.nz;
+    *grid = ctx->trace_grid;
+    if (!out) return SHG_OK;
+    if (!ctx->d_trace || ctx->trace_grid == 0) return SHG_ESTATE;
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    CU(cudaMemcpy(out, ctx->d_trace, sizeof(long long) * (size_t)(*steps) * ctx->trace_grid * 8, cudaMemcpyDeviceToHost));
     return SHG_OK;
 }
 

@@ -562,10 +562,11 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
 
 // Monotonic-counter barrier: instance k is complete when the counter reaches (k+1) * gridDim.x.
 // A bounded spin turns a lost CTA into an error status instead of a hung GPU.
-__device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch) {
+__device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch, int n, int which) {
     __shared__ int ok;
     __syncthreads();
     if (threadIdx.x == 0) {
+        const long long t_cta = clock64();
         epoch += 1;
         const unsigned int target = epoch * gridDim.x;
         __threadfence();
@@ -578,6 +579,14 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         }
         __threadfence();
         ok = good;
+        if (P.trace != nullptr && n < P.trace_steps) {
+            long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
+            unsigned long long gt;
+            unsigned int smid;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            t[0] = t_cta; t[1] = clock64(); t[2] = (long long)gt; t[3] = (long long)smid;
+        }
     }
     __syncthreads();
     return ok != 0;
@@ -594,9 +603,9 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         row_pass<N, ROW_MID, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
-        if (!grid_barrier(P, epoch)) return;
+        if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC>(P, hsel, smem_cta, tws, warp, lane);
-        if (!grid_barrier(P, epoch)) return;
+        if (!grid_barrier(P, epoch, n, 1)) return;
     }
 }
 

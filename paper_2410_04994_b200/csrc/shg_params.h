@@ -36,6 +36,8 @@ struct Params {
     double* hist;              // [batch][nz+1][2]
     unsigned int* barrier;     // grid barrier counter (persistent kernel)
     int* status;               // device status word (barrier timeout)
+    long long* trace;          // optional phase timeline of the persistent kernel (SHG_OPT_TRACE), else null:
+    int trace_steps;           //   [trace_steps][grid][2 barriers][4] = {clock64 CTA done, clock64 grid done, globaltimer, smid}
 };
 
 enum RowMode { ROW_FIRST = 0, ROW_MID = 1, ROW_FINAL = 2 };

@@ -15,11 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libshg.so")
 
 SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
-OPT_PERSISTENT, OPT_PRECISE = 1, 2
+OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE = 1, 2, 3
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_power", "shg_power_history", "shg_gaussian_input",
-           "shg_enable_timing", "shg_last_main_loop_ms", "shg_last_launch_count", "shg_destroy", "shg_strerror")
+           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_last_launch_count", "shg_destroy", "shg_strerror")
 
 
 class Grid(C.Structure):
@@ -66,6 +66,7 @@ def lib():
     L.shg_gaussian_input.argtypes = [vp, vp, C.c_int, vp]
     L.shg_enable_timing.argtypes = [vp, C.c_int]
     L.shg_last_main_loop_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.shg_read_trace.argtypes = [vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.shg_last_launch_count.argtypes = [vp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
@@ -232,6 +233,14 @@ class Shg:
         ms = C.c_float()
         _check(lib().shg_last_main_loop_ms(self._h, C.byref(ms)))
         return float(ms.value)
+
+    def read_trace(self) -> np.ndarray:
+        """int64 [steps][grid][2][4] phase timeline (see SHG_OPT_TRACE in include/shg.h)."""
+        steps, grid = C.c_int(), C.c_int()
+        _check(lib().shg_read_trace(self._h, None, C.byref(steps), C.byref(grid)))
+        out = np.zeros((steps.value, grid.value, 2, 4), dtype=np.int64)
+        _check(lib().shg_read_trace(self._h, C.c_void_p(out.ctypes.data), C.byref(steps), C.byref(grid)))
+        return out
 
     def last_launch_count(self) -> int:
         return int(lib().shg_last_launch_count(self._h))
