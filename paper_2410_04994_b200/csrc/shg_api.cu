@@ -106,6 +106,7 @@ struct shg_ctx {
     long long* d_trace = nullptr;
     int trace_steps = 0;        // steps recorded per propagate (0 = tracing off)
     int trace_grid = 0;         // CTAs of the last traced launch
+    int stagger_row = 0, stagger_col = 0;
 
     const float* d_T = nullptr;
     double T_uniform = 0.0;
@@ -329,6 +330,8 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
         case SHG_OPT_PRECISE:
             if (ctx->precise != (value != 0)) { ctx->precise = (value != 0); ctx->tables_dirty = true; }
             return SHG_OK;
+        case 100: ctx->stagger_row = value; return SHG_OK;
+        case 101: ctx->stagger_col = value; return SHG_OK;
         case SHG_OPT_TRACE: {
             if (value < 0 || value > 4096) return SHG_EINVAL;
             if (value != ctx->trace_steps) {
@@ -404,6 +407,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.barrier = ctx->d_barrier;
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
     P.trace = ctx->d_trace;
+    P.stagger_row = ctx->stagger_row; P.stagger_col = ctx->stagger_col;
     P.trace_steps = ctx->trace_steps;
 
     const size_t np = np_of(ctx);

@@ -101,6 +101,19 @@ __device__ __forceinline__ const float4* ptr_after(const float4* p, float dep) {
     return r;
 }
 
+// Pull one line group's table (N float4 = N/8 lines of 128 B) into L1: the device-wide barrier's fence
+// invalidates L1 every pass, and the chained table loads below would otherwise each pay an L2 round trip.
+template <int R, int M>
+__device__ __forceinline__ void table_prefetch(const float4* __restrict__ tab, int m) {
+    constexpr int LINES = R * M / 8, PER_LANE = (LINES + M - 1) / M;
+#pragma unroll
+    for (int i = 0; i < PER_LANE; ++i) {
+        const int line = m + M * i;
+        if (LINES % M == 0 || line < LINES)
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(tab + 8 * line));
+    }
+}
+
 // v[q] *= table[M q] for q = 0..R-1 (table already offset by the lane), loads chained TABLE_DEPTH deep
 template <int R, int M, bool PREC, bool CONJ_OUT>
 __device__ __forceinline__ void table_mul(float2 (&v)[R], const float4* __restrict__ tab) {
@@ -338,30 +351,41 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 
     if constexpr (MODE == ROW_MID) {
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
+        const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
-        // temperature / phase operands of the first RK4 point are requested before the transform
+        table_prefetch<R, M>(hx, m);
+        // temperature / phase operands of the first RK4 point are requested before the transform (when
+        // registers allow), those of the second right after it; inside the loop two points ahead
         const size_t plane = (size_t)P.ny * NX;
         const size_t pbase = (size_t)y * NX + rot + m;
         const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
         const float* Ta = nullptr;
         const float* Tn = nullptr;
         float* phi = nullptr;
-        TPoint cur{};
+        TPoint cur{}, nxt{};
         if (P.nzt != 0) {
             const float* Tb = P.T + (P.T_per_member ? (size_t)b * P.nzt * plane : 0);
             Ta = Tb + (size_t)ta.k * plane;
             Tn = Tb + (size_t)tb.k * plane;
             phi = P.phi + (size_t)b * plane + pbase;
-            cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
+            if constexpr (R < 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
         }
         warp_fft<NX, PREC>(v, own, tws, m);
+        if (P.nzt != 0) {
+            // (a 32-value line leaves no registers to carry operands across the transform)
+            if constexpr (R >= 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
+            nxt = t_load(Ta, Tn, plane, pbase + M, ta.two, tb.two, phi + M);
+        }
         // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2)
 #pragma unroll
         for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
 
-        // ---- nonlinear step on elements e = M q + m + f N/2, q < R/2: own lower half, partner's upper half
+        // ---- nonlinear step on elements e = M q + m + f N/2, q < R/2: own lower half, partner's upper half.
+        // p1 / p2 address A1 / A2 of this lane's points whichever side it is on (no value selects).
+        float2* p1 = (f ? par + M * H : own) + m;
+        float2* p2 = (f ? own : par + M * H) + m;
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz, g1 = mb.g1dz, g2 = mb.g2dz;
         float s1 = 0.f, s2 = 0.f;
         if (P.nzt == 0) {
@@ -381,25 +405,25 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                             CB = phase_coef(cb, sb, k1dz, k2dz);
 #pragma unroll 2
             for (int q = 0; q < H; ++q) {
-                const float2 o = own[M * q + m], p = par[M * (q + H) + m];
-                float2 a1 = f ? p : o, a2 = f ? o : p;
+                float2 a1 = p1[M * q], a2 = p2[M * q];
                 a1.y = -a1.y; a2.y = -a2.y;
                 rk4_point(a1, a2, CA, CM, CB, g1, g2);
                 s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
                 s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
-                own[M * q + m] = f ? a2 : a1;
-                par[M * (q + H) + m] = f ? a1 : a2;
+                p1[M * q] = a1;
+                p2[M * q] = a2;
             }
         } else {
             const float hdz = 0.5f * mb.dz, e8 = 0.125f * mb.dz;
-#pragma unroll 2
-            for (int q = 0; q < H; ++q) {
-                const TPoint tp = cur;
-                if (q + 1 < H) cur = t_load(Ta, Tn, plane, pbase + M * (q + 1), ta.two, tb.two, phi + M * (q + 1));
-                float dTa = dT_lerp(tp.a0, tp.a1, ta.f, ta.two, mb.Tpm_hi, mb.Tpm_lo);
-                float dTb = dT_lerp(tp.b0, tp.b1, tb.f, tb.two, mb.Tpm_hi, mb.Tpm_lo);
-                float dka = fmaf(mb.gT, dTa, mb.dk0), dkb = fmaf(mb.gT, dTb, mb.dk0);
-                float ph = tp.ph;
+            const float gT = mb.gT, dk0 = mb.dk0, Thi = mb.Tpm_hi, Tlo = mb.Tpm_lo;
+            // one point: consume operands tp (requested two points earlier), request those of point q + 2
+            auto point = [&](int q, TPoint& tp) {
+                const float a0 = tp.a0, a1v = tp.a1, b0 = tp.b0, b1 = tp.b1, ph = tp.ph;
+                const int qn = (q + 2 < H) ? q + 2 : H - 1;          // clamped: the tail re-reads, never branches
+                tp = t_load(Ta, Tn, plane, pbase + M * qn, ta.two, tb.two, phi + M * qn);
+                float dTa = dT_lerp(a0, a1v, ta.f, ta.two, Thi, Tlo);
+                float dTb = dT_lerp(b0, b1, tb.f, tb.two, Thi, Tlo);
+                float dka = fmaf(gT, dTa, dk0), dkb = fmaf(gT, dTb, dk0);
                 float phm = fmaf(e8, fmaf(3.0f, dka, dkb), ph);        // phi_n + dz (3 dk_n + dk_{n+1})/8
                 float phb = fmaf(hdz, dka + dkb, ph);                  // phi_n + dz (dk_n + dk_{n+1})/2
                 float ca, sa, cm, sm, cb, sb;
@@ -409,14 +433,18 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                 __stcg(phi + M * q, wrap_2pi(phb));
                 const PhaseCoef CA = phase_coef(ca, sa, k1dz, k2dz), CM = phase_coef(cm, sm, k1dz, k2dz),
                                 CB = phase_coef(cb, sb, k1dz, k2dz);
-                const float2 o = own[M * q + m], p = par[M * (q + H) + m];
-                float2 a1 = f ? p : o, a2 = f ? o : p;
+                float2 a1 = p1[M * q], a2 = p2[M * q];
                 a1.y = -a1.y; a2.y = -a2.y;
                 rk4_point(a1, a2, CA, CM, CB, g1, g2);
                 s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
                 s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
-                own[M * q + m] = f ? a2 : a1;
-                par[M * (q + H) + m] = f ? a1 : a2;
+                p1[M * q] = a1;
+                p2[M * q] = a2;
+            };
+#pragma unroll 1
+            for (int q = 0; q < H; q += 2) {
+                point(q, cur);
+                point(q + 1, nxt);
             }
         }
         s1 = warp_sum(s1); s2 = warp_sum(s2);
@@ -430,61 +458,104 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
-        table_mul<R, M, PREC, false>(v, P.hx[hsel] + ((size_t)b * 2 + f) * NX + m);
+        table_mul<R, M, PREC, false>(v, hx + m);
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// Column pass, one item = a strip of SC adjacent columns of one field of one member, handled by a team of
-// TW warps:  stage the strip in shared memory (64 B per row, coalesced) -> F_y -> * hy (includes 1/(nx ny)),
-// conjugated -> F_y -> stage out.  The strip is held column by column, so each column is a line the
-// transform can transpose in place.
+// Forward transform of SC = 8 adjacent columns by a team of TW = M/4 warps ("tile" layout).  Thread
+// (c, t) -- lane = 8 j + c, t = 4 (warp rank in team) + j -- holds, for column c, the elements t + M q,
+// q = 0..R-1, in v[q]: the same strided layout in and out as warp_fft, but the M residues of a column sit
+// in M different (c, t) threads spread over the team instead of in the M lanes of one warp.  Hence
+//   * a load / store of v[q] touches 4 consecutive rows x 64 contiguous bytes: the strip needs no staging;
+//   * the twiddle W_N^{t k1} depends on the lane only through j: a 128-bit table read is a 4-address
+//     broadcast (one wavefront instead of four);
+//   * the one transpose goes through the strip's shared-memory tile with two team barriers.
+// col: the strip's tile, one padded line of pitch CP per column (conflict free for both access patterns:
+// CP = 2 mod 16, M + 1 odd).
 // ------------------------------------------------------------------------------------------------
-template <int NY, bool PREC>
+template <int N, bool PREC>
+__device__ __forceinline__ void tile_fft(float2 (&v)[FftCfg<N>::R], float2* __restrict__ colline,
+                                         const float4* __restrict__ tws, int t, int bar_id) {
+    constexpr int R = FftCfg<N>::R, M = FftCfg<N>::M, Q = R / M, MP = M + 1, TT = Geo<N>::TW * 32;
+    const unsigned tws_saddr = (unsigned)__cvta_generic_to_shared(tws + t);
+    float2* wr = colline + t;            // value (k1, residue t) goes to slot k1 * MP + t ...
+    float2* rd = colline + t * MP;       // ... and thread t collects row k1 = t (+ M i): slots k1 * MP + n2
+    if constexpr (Q == 1) {
+#pragma unroll 1
+        for (int s = 0; s < 2; ++s) {
+            fft_reg<R, false, PREC>(v);
+            if (s == 0) {
+                twiddle_all<N, PREC>(v, tws_saddr, std::make_integer_sequence<int, R - 1>{});
+                named_barrier(bar_id, TT);              // every reader of the previous exchange is done
+#pragma unroll
+                for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
+                named_barrier(bar_id, TT);
+#pragma unroll
+                for (int n2 = 0; n2 < M; ++n2) v[n2] = rd[n2];
+            }
+        }
+    } else {
+        fft_reg<R, false, PREC>(v);
+        twiddle_all<N, PREC>(v, tws_saddr, std::make_integer_sequence<int, R - 1>{});
+        named_barrier(bar_id, TT);
+#pragma unroll
+        for (int k1 = 0; k1 < R; ++k1) wr[k1 * MP] = v[k1];
+        named_barrier(bar_id, TT);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            float2 u[M];
+#pragma unroll
+            for (int n2 = 0; n2 < M; ++n2) u[n2] = rd[i * M * MP + n2];
+            fft_reg<M, false, PREC>(u);
+#pragma unroll
+            for (int k2 = 0; k2 < M; ++k2) v[i + Q * k2] = u[k2];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Column pass, one item = a strip of SC = 8 adjacent columns of one field of one member, handled by a team
+// of TW warps:  load (4 rows x 64 B per warp instruction) -> F_y -> * hy (includes 1/(nx ny)), conjugated
+// -> F_y -> store to the same addresses.
+// ------------------------------------------------------------------------------------------------
+// NXC: the row length when it is known at compile time (square grids in the persistent kernel: every
+// load / store is then one base register plus an immediate), 0 = take P.nx.
+template <int NY, bool PREC, int NXC>
 __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, float2* strip,
                                          const float4* __restrict__ tws, int trank, int bar_id, int lane) {
     using GE = Geo<NY>;
-    constexpr int R = GE::R, M = GE::M, G = GE::G, SC = GE::SC, CP = GE::CP, TT = GE::TW * 32;
-    const int nx = P.nx;
+    constexpr int R = GE::R, M = GE::M, SC = GE::SC, CP = GE::CP;
+    static_assert(SC == 8 && GE::TW * 4 == M, "tile layout: 8 columns x 4 residues per warp");
+    const int nx = NXC ? NXC : P.nx;
     const int strips_per_field = nx / SC;
     const int bf = item / strips_per_field;                   // b*2 + f
     const int c0 = (item - bf * strips_per_field) * SC;
-    const int t = trank * 32 + lane;
-    // staging: thread t moves elements (row, column) = (t / SC + i TT / SC, t % SC), i = 0..R-1
-    float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + c0 + (size_t)(t / SC) * nx + (t % SC);
-    const size_t gstep = (size_t)(TT / SC) * nx;
-    float2* st = strip + (t % SC) * CP + (t / SC);
+    const int c = lane & 7, t = trank * 4 + (lane >> 3);
+    float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + c0 + c + (size_t)t * nx;
+    const size_t gstep = (size_t)M * nx;
     const float4* h = P.hy[hsel] + (size_t)bf * NY;
+    float2* colline = strip + c * CP;
     float2 v[R];
 
 #pragma unroll
-    for (int i = 0; i < R; ++i) v[i] = ldcg2(A + i * gstep);
+    for (int q = 0; q < R; ++q) v[q] = ldcg2(A + q * gstep);
+    table_prefetch<R, M>(h, t);
+    tile_fft<NY, PREC>(v, colline, tws, t, bar_id);
+    table_mul<R, M, PREC, true>(v, h + t);
+    tile_fft<NY, PREC>(v, colline, tws, t, bar_id);
+    if constexpr (NXC == 0) {
+        // runtime stride: recompute the addresses instead of keeping R pointers alive across the transforms
+        asm volatile("" : "+l"(A));
+        float2* a = A;
 #pragma unroll
-    for (int i = 0; i < R; ++i) st[i * (TT / SC)] = v[i];
-    named_barrier(bar_id, TT);
-
-    // lane group g of warp trank owns one column; with four groups per warp the two groups that share a
-    // wavefront take columns 4 apart (their lines then start 16 banks apart)
-    const int g = lane / M, m = lane % M;
-    const int cg = (G == 4) ? (trank * 2 + (g >> 1) + 4 * (g & 1)) : (trank * G + g);
-    float2* line = strip + cg * CP;
+        for (int q = 0; q < R; ++q) { stcg2(a, v[q]); a += gstep; }
+    } else {
 #pragma unroll
-    for (int q = 0; q < R; ++q) v[q] = line[M * q + m];
-    __syncwarp();
-    warp_fft<NY, PREC>(v, line, tws, m);
-    table_mul<R, M, PREC, true>(v, h + m);
-    warp_fft<NY, PREC>(v, line, tws, m);
-#pragma unroll
-    for (int q = 0; q < R; ++q) line[M * q + m] = v[q];
-    named_barrier(bar_id, TT);
-
-    // stage out (each thread reads back exactly the elements it will overwrite at the next stage-in)
-#pragma unroll
-    for (int i = 0; i < R; ++i) v[i] = st[i * (TT / SC)];
-#pragma unroll
-    for (int i = 0; i < R; ++i) stcg2(A + i * gstep, v[i]);
+        for (int q = 0; q < R; ++q) stcg2(A + q * gstep, v[q]);
+    }
 }
 
 template <int NX> __host__ __device__ inline int row_items(int batch, int ny) { return batch * ny / Geo<NX>::HG; }
@@ -513,11 +584,12 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
     cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
     if (slot >= P.row_slots) return;
+    if (P.stagger_row > 0 && (slot & 1)) { const long long t0 = clock64(); while (clock64() - t0 < P.stagger_row) {} }
     for (int it = lo + slot; it < hi; it += P.row_slots)
         row_item<NX, MODE, PREC>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
 
-template <int NY, bool PREC>
+template <int NY, bool PREC, int NXC>
 __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane) {
     using GE = Geo<NY>;
@@ -526,8 +598,9 @@ __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem
     const int team = warp / GE::TW, trank = warp % GE::TW;
     float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
     if (team >= P.col_teams) return;
+    if (P.stagger_col > 0 && (team & 1)) { const long long t0 = clock64(); while (clock64() - t0 < P.stagger_col) {} }
     for (int it = lo + team; it < hi; it += P.col_teams)
-        col_item<NY, PREC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
+        col_item<NY, PREC, NXC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -546,7 +619,7 @@ __global__ void __launch_bounds__(Geo<NY>::THREADS, 1) k_col(Params P, int hsel)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<NY>(smem_raw, P.twy);
-    col_pass<NY, PREC>(P, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
+    col_pass<NY, PREC, 0>(P, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -554,14 +627,16 @@ __global__ void __launch_bounds__(Geo<NY>::THREADS, 1) k_col(Params P, int hsel)
 // dependency is one barrier between a row pass and a column pass (a 2-D FFT needs every row before any
 // column).  Launched cooperatively (all CTAs co-resident), one CTA per SM.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
     unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 
 // Monotonic-counter barrier: instance k is complete when the counter reaches (k+1) * gridDim.x.
-// A bounded spin turns a lost CTA into an error status instead of a hung GPU.
+// Arrive = one release reduction (orders the whole CTA's stores, which thread 0 observed through
+// bar.sync, before the increment; no value returned, so no round trip), poll = relaxed loads, then ONE
+// acquire fence.  A bounded spin turns a lost CTA into an error status instead of a hung GPU.
 __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch, int n, int which) {
     __shared__ int ok;
     __syncthreads();
@@ -569,15 +644,16 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         const long long t_cta = clock64();
         epoch += 1;
         const unsigned int target = epoch * gridDim.x;
-        __threadfence();
-        atomicAdd(P.barrier, 1u);
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(P.barrier), "r"(1u) : "memory");
         int good = 1;
-        long long t0 = clock64();
-        while (ld_acquire_u32(P.barrier) < target) {
-            if (clock64() - t0 > 4000000000LL) { good = 0; atomicExch(P.status, 1); break; }
-            if (*((volatile int*)P.status) != 0) { good = 0; break; }
+        if (ld_relaxed_u32(P.barrier) < target) {
+            const long long t0 = clock64();
+            while (ld_relaxed_u32(P.barrier) < target) {
+                if (clock64() - t0 > 4000000000LL) { good = 0; atomicExch(P.status, 1); break; }
+                if (*((volatile int*)P.status) != 0) { good = 0; break; }
+            }
         }
-        __threadfence();
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
         ok = good;
         if (P.trace != nullptr && n < P.trace_steps) {
             long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
@@ -604,7 +680,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         row_pass<N, ROW_MID, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC>(P, hsel, smem_cta, tws, warp, lane);
+        col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;
     }
 }
