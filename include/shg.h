@@ -83,6 +83,10 @@ typedef struct {
                                   (0 = after the row pass, 1 = after the column pass) four int64: SM clock when
                                   the CTA finished its share of the pass, SM clock when the barrier released it,
                                   %globaltimer (ns) at release, SM id.  Read back with shg_read_trace.            */
+#define SHG_OPT_ACQUIRE_FENCE 4 /* persistent kernel.  0 (default): after a device-wide barrier the fields are read
+                                  with L2-only loads (ld.global.cg) and no fence is issued; 1: additionally issue a
+                                  gpu-scope acquire fence (invalidates L1) after every barrier, as the letter of
+                                  the PTX memory model asks.  Bit-identical results; ~350 SM clocks per barrier.   */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);

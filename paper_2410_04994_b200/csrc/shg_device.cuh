@@ -635,8 +635,9 @@ __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
 
 // Monotonic-counter barrier: instance k is complete when the counter reaches (k+1) * gridDim.x.
 // Arrive = one release reduction (orders the whole CTA's stores, which thread 0 observed through
-// bar.sync, before the increment; no value returned, so no round trip), poll = relaxed loads, then ONE
-// acquire fence.  A bounded spin turns a lost CTA into an error status instead of a hung GPU.
+// bar.sync, before the increment; no value returned, so no round trip), poll = relaxed loads (one L2 round
+// trip per poll; the timeout / status checks only every 32nd).  A bounded spin turns a lost CTA into an
+// error status instead of a hung GPU.
 __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch, int n, int which) {
     __shared__ int ok;
     __syncthreads();
@@ -648,12 +649,22 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         int good = 1;
         if (ld_relaxed_u32(P.barrier) < target) {
             const long long t0 = clock64();
+            int spins = 0;
             while (ld_relaxed_u32(P.barrier) < target) {
-                if (clock64() - t0 > 4000000000LL) { good = 0; atomicExch(P.status, 1); break; }
-                if (*((volatile int*)P.status) != 0) { good = 0; break; }
+                // (the timeout / status checks cost an L2 round trip: not in every poll)
+                if (((++spins) & 31) == 0) {
+                    if (clock64() - t0 > 4000000000LL) { good = 0; atomicExch(P.status, 1); break; }
+                    if (*((volatile int*)P.status) != 0) { good = 0; break; }
+                }
             }
         }
-        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+        // Acquire side.  Every mutable global array (fields, phi) is read with ld.global.cg (SASS: LDG.STRONG.GPU,
+        // served by L2, never by L1) by threads that pass the bar.sync below only after this poll has
+        // observed the last arrival, whose red.release ordered that CTA's stores before it; the arrays that
+        // L1 may hold (tables, T, member constants) are read-only during a propagate.  A gpu-scope fence here
+        // (MEMBAR + L1 invalidation, ~350 clocks per barrier and cold tables every pass) is therefore only
+        // needed by the letter of the PTX model: SHG_OPT_ACQUIRE_FENCE = 1 turns it on (bit-identical results).
+        if (P.acquire_fence) asm volatile("fence.acq_rel.gpu;" ::: "memory");
         ok = good;
         if (P.trace != nullptr && n < P.trace_steps) {
             long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
