@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libshg.so")
 SIZES = (64, 128, 256, 512, 1024)
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-         "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
+         "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + os.environ.get("SHG_NVCC_EXTRA", "").split()
 
 
 def _sources():

@@ -108,8 +108,12 @@ __device__ __forceinline__ void dif_bfly(float2 (&v)[R]) {
     constexpr int i0 = grp * 2 * SPAN + k, i1 = i0 + SPAN;
     constexpr int E = k * (16 / SPAN);       // W_{2 SPAN}^k = W_32^{k 16/SPAN}
     float2 a = v[i0], b = v[i1];
-    v[i0] = make_float2(a.x + b.x, a.y + b.y);
-    v[i1] = twmul32<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));
+    // Blackwell packed fp32x2 adds (FADD2: one issue slot for the re and im lanes of a register pair; the
+    // negation is an operand modifier).  The -i twiddle swaps re and im, which a register pair cannot do for
+    // free, so that difference stays scalar (its swap is then just register naming).
+    v[i0] = __fadd2_rn(a, b);
+    if constexpr (E == 8) v[i1] = twmul32<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));
+    else v[i1] = twmul32<E, INV, PREC>(__fadd2_rn(a, make_float2(-b.x, -b.y)));
 }
 
 template <int R, int SPAN, bool INV, bool PREC, int... J>
