@@ -140,6 +140,11 @@ int shg_last_main_loop_ms(shg_ctx* ctx, float* ms);
  * Synchronises the stream of the last propagate. */
 int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid);
 
+/* Measured fp32 pipe peak of the current device: a register-only FFMA kernel (16 independent chains per
+ * thread, 512 threads per SM) timed with CUDA events.  *tflops receives 2 flops per FFMA lane-op over the
+ * elapsed time.  It is the denominator of bench.py's "alu" roofline (nominal: SMs x 128 lanes x 2 x clock). */
+int shg_measure_fp32_peak(double* tflops);
+
 /* Number of kernels the last shg_propagate / shg_propagate_host launched. */
 int shg_last_launch_count(const shg_ctx* ctx);
 

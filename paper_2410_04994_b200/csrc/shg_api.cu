@@ -76,6 +76,22 @@ __global__ void k_gaussian(float2* A, const shg::GaussDev* gd, int nx, int ny, i
     A[i] = make_float2(mag * (g.ar * c - g.ai * s), mag * (g.ar * s + g.ai * c));
 }
 
+// fp32 pipe peak: 16 independent FFMA chains per thread, nothing else in the loop
+__global__ void __launch_bounds__(512, 1) k_fp32_peak(float* out, const float* in, int iters) {
+    float a[16];
+    const float b = in[threadIdx.x & 31], c = in[32 + (threadIdx.x & 31)];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = in[i] + (float)threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], b, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace
 
 struct shg_ctx {
@@ -577,6 +593,37 @@ int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid) {
     if (!ctx->d_trace || ctx->trace_grid == 0) return SHG_ESTATE;
     CU(cudaStreamSynchronize(ctx->last_stream));
     CU(cudaMemcpy(out, ctx->d_trace, sizeof(long long) * (size_t)(*steps) * ctx->trace_grid * 8, cudaMemcpyDeviceToHost));
+    return SHG_OK;
+}
+
+int shg_measure_fp32_peak(double* tflops) {
+    if (!tflops) return SHG_EINVAL;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float *out = nullptr, *in = nullptr;
+    CU(cudaMalloc((void**)&out, sizeof(float) * (size_t)sms * 512));
+    CU(cudaMalloc((void**)&in, 4096));
+    CU(cudaMemset(in, 0, 4096));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int iters = 20000;
+    float best = 0.f;
+    for (int rep = 0; rep < 4; ++rep) {        // first repetition warms up
+        CU(cudaEventRecord(e0, nullptr));
+        k_fp32_peak<<<sms, 512>>>(out, in, iters);
+        CU(cudaEventRecord(e1, nullptr));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && (best == 0.f || ms < best)) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    cudaFree(in);
+    *tflops = 2.0 * 16.0 * (double)iters * 512.0 * (double)sms / ((double)best * 1e-3) / 1e12;
     return SHG_OK;
 }
 

@@ -19,7 +19,7 @@ OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE = 1, 2, 3, 4
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_power", "shg_power_history", "shg_gaussian_input",
-           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_last_launch_count", "shg_destroy", "shg_strerror")
+           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak", "shg_last_launch_count", "shg_destroy", "shg_strerror")
 
 
 class Grid(C.Structure):
@@ -68,6 +68,7 @@ def lib():
     L.shg_last_main_loop_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.shg_read_trace.argtypes = [vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.shg_last_launch_count.argtypes = [vp]
+    L.shg_measure_fp32_peak.argtypes = [dp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
     L.shg_strerror.argtypes = [C.c_int]
@@ -105,6 +106,13 @@ def _dev_ptr(t, dtype_names):
     if str(t.dtype).replace("torch.", "") not in dtype_names:
         raise TypeError("expected dtype in %s, got %s" % (dtype_names, t.dtype))
     return C.c_void_p(t.data_ptr())
+
+
+def measure_fp32_peak() -> float:
+    """Measured fp32 FFMA peak of the current device in TFLOP/s (shg_measure_fp32_peak)."""
+    v = C.c_double()
+    _check(lib().shg_measure_fp32_peak(C.byref(v)))
+    return float(v.value)
 
 
 class Shg:
