@@ -61,6 +61,7 @@ def _load():
                                C.POINTER(C.c_void_p)]
     lib.orc_set_temperature.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_int]
     lib.orc_propagate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+    lib.orc_set_heat_output.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.orc_power.argtypes = [C.c_void_p, C.c_int, C.c_double, dp, dp]
     lib.orc_power_history.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
     lib.orc_destroy.argtypes = [C.c_void_p]
@@ -138,6 +139,7 @@ class Oracle:
             raise ValueError("orc_create failed: %d" % rc)
         self._h = h
         self._T = None
+        self._Q = None
 
     def set_temperature(self, T=None, T_uniform: float = 0.0, per_member: bool = False):
         ptr = None
@@ -152,6 +154,19 @@ class Oracle:
         if rc:
             raise ValueError("orc_set_temperature failed: %d" % rc)
         return self
+
+    def set_heat_output(self, nq: int):
+        """Ask the next propagate for the heat source of P:118 (Eq. 8) on nq planes; returns the float64 array
+        [batch][nq][ny][nx] that the propagate fills (nq = 0 switches it off)."""
+        if nq <= 0:
+            self._Q = None
+            rc = _load().orc_set_heat_output(self._h, None, 0)
+        else:
+            self._Q = np.zeros((self.grid["batch"], nq, self.grid["ny"], self.grid["nx"]), dtype=np.float64)
+            rc = _load().orc_set_heat_output(self._h, self._Q.ctypes.data, int(nq))
+        if rc:
+            raise ValueError("orc_set_heat_output failed: %d" % rc)
+        return self._Q
 
     def propagate(self, A1, A2=None):
         ny, nx = self.grid["ny"], self.grid["nx"]

@@ -46,6 +46,8 @@ struct orc_ctx {
     int         T_set;
     double*     hist;        /* [batch][nz+1][2] */
     int         propagated;
+    double*     Q;           /* borrowed heat-source output [batch][nq][ny][nx], or NULL */
+    int         nq;
 };
 
 int orc_num_threads(void) {
@@ -207,6 +209,14 @@ void orc_destroy(orc_ctx* ctx) {
     free(ctx);
 }
 
+int orc_set_heat_output(orc_ctx* ctx, double* Q, int nq) {
+    if (!ctx) return -1;
+    if (Q && (nq < 1 || nq > ctx->g.nz)) return -1;
+    ctx->Q = Q;
+    ctx->nq = Q ? nq : 0;
+    return 0;
+}
+
 int orc_set_temperature(orc_ctx* ctx, const float* T, double T_uniform, int per_member) {
     if (!ctx) return -1;
     if (ctx->g.nzt > 0 && !T) return -1;
@@ -270,6 +280,13 @@ static inline void rk4_point(const nl_par* p, cplx* A1, cplx* A2, double h,
 
 /* Factor of the linear step of length h for one field (P:143 L_j; P:346-352 Eq. A.4-A.5; sign G3):
  *   Hj[my][mx] = exp(-i (kx^2+ky^2) h / (2 k_j) - alpha_j h / 2),  kx = 2 pi m'/lx, m' = m or m-nx (G11) */
+/* q = sum_j alpha_j I_j + beta_j I_j^2,  I_j = eps0 c n_j |A_j|^2 / 2   (Eq. 8) */
+static inline double heat_source(const nl_par* p, const orc_crystal* c, cplx A1, cplx A2) {
+    double I1 = p->c1 * (creal(A1) * creal(A1) + cimag(A1) * cimag(A1));
+    double I2 = p->c2 * (creal(A2) * creal(A2) + cimag(A2) * cimag(A2));
+    return c->alpha1 * I1 + c->beta1 * I1 * I1 + c->alpha2 * I2 + c->beta2 * I2 * I2;
+}
+
 static cplx* linear_factor(const orc_grid* g, const orc_beam* bm, double kj, double alpha, double h) {
     int nx = g->nx, ny = g->ny;
     cplx* H = (cplx*)malloc(sizeof(cplx) * (size_t)nx * ny);
@@ -354,6 +371,20 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
             /* L/2 */
             linear_step(A1, g, H1, brute, parallel);
             linear_step(A2, g, H2, brute, parallel);
+            /* heat source of Eq. 8, plane k <- z-step n_k = floor((2k+1) nz/(2 nq)): mean of the source
+             * on the real-space fields before and after the nonlinear step (both sit at z_n + dz/2 as far as
+             * the linear part goes; the mean is the trapezoid rule over the nonlinear step), G27 */
+            double* qplane = NULL;
+            if (ctx->Q) {
+                for (int k = 0; k < ctx->nq; ++k) {
+                    long long nk = ((2LL * k + 1) * nz) / (2LL * ctx->nq);
+                    if (nk > nz - 1) nk = nz - 1;
+                    if (nk == n) qplane = ctx->Q + ((size_t)b * ctx->nq + k) * np;
+                }
+            }
+            if (qplane) {
+                for (size_t i = 0; i < np; ++i) qplane[i] = heat_source(&p, c, A1[i], A2[i]);
+            }
             /* N(dz), one RK4 step per point */
 #pragma omp parallel for schedule(static) if (parallel)
             for (long long i = 0; i < (long long)np; ++i) {
@@ -364,6 +395,10 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
                 double ph_b = phase_at(phi[i], dk_n, dk_n1, dz, dz);
                 rk4_point(&p, &A1[i], &A2[i], dz, ph_a, ph_m, ph_b);
                 phi[i] = ph_b;
+            }
+            /* heat source of Eq. 8 on the planes whose sampled step is n: second half of the mean (G27) */
+            if (qplane) {
+                for (size_t i = 0; i < np; ++i) qplane[i] = 0.5 * (qplane[i] + heat_source(&p, c, A1[i], A2[i]));
             }
             /* L/2 */
             linear_step(A1, g, H1, brute, parallel);

@@ -73,6 +73,13 @@ int  orc_propagate(orc_ctx*, const double* A1_in, const double* A2_in, double* A
                    int batch);
 /* Power (W) of both fields of one member at the recorded node nearest to z.  P:120 (I).      */
 int  orc_power(orc_ctx*, int member, double z, double* P1, double* P2);
+/* Internal heat source of P:118 (Eq. 8), q = sum_j alpha_j I_j + beta_j I_j^2 with I_j = eps0 c n_j |A_j|^2/2
+ * (P:120), sampled on nq (1 <= nq <= nz) planes along z: plane k holds the mean of q evaluated on the
+ * real-space fields right before and right after the nonlinear step of z-step n_k = floor((2k+1) nz / (2 nq)),
+ * i.e. q at z = z_{n_k} + dz/2 to second order in dz (the middle of the cell [k L/nq, (k+1) L/nq) rounded to
+ * a step; reading G27 in DESIGN.md: the paper does not say where along a step the source is taken).  Q: host double [batch][nq][ny][nx], borrowed, filled by the next
+ * orc_propagate (scheme 0 only); NULL switches it off.                                                */
+int  orc_set_heat_output(orc_ctx*, double* Q, int nq);
 /* Whole history of one member: out[(nz+1)][2] = {P1(z_n), P2(z_n)}, n = 0..nz.                       */
 int  orc_power_history(orc_ctx*, int member, double* out);
 void orc_destroy(orc_ctx*);

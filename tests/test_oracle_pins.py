@@ -430,3 +430,64 @@ def test_workload_generator_matches_oracle_eq6_and_sizes():
     w4 = wl.make("cfg4", nz=4)
     assert len(w4["beams"]) == 64 and w4["A1"].shape == (64, 128, 128)
     assert abs(w4["beams"][0]["w0"] - 108.9e-6) < 0.1e-6 and abs(w4["beams"][63]["w0"] - 15.4e-6) < 0.05e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# 13. heat source of Eq. 8, S§8(f) rank 1: closed forms for its two terms, plane placement (G27),
+#     and the energy balance (what the fields lose is what the crystal absorbs)
+# ------------------------------------------------------------------------------------------------
+def q_steps(nz, nq):
+    return [min(nz - 1, ((2 * k + 1) * nz) // (2 * nq)) for k in range(nq)]
+
+
+def test_heat_source_linear_absorption_closed_form_and_plane_placement():
+    A0, a1, a2 = 3e6, 4.0, 9.0
+    g, c, bm, A1 = plane_wave_case(A0, nz=60, d_eff=0.0, alpha1=a1, alpha2=a2)
+    dz = c["L"] / g["nz"]
+    for nq in (60, 7, 1):
+        o = oracle.Oracle(g, c, [bm])
+        Q = o.set_heat_output(nq)
+        o.propagate(A1, 0.5 * A1)
+        I1 = EPS0 * C0 * c["n1"] * A0 ** 2 / 2
+        I2 = EPS0 * C0 * c["n2"] * (0.5 * A0) ** 2 / 2
+        zq = (np.array(q_steps(g["nz"], nq)) + 0.5) * dz           # the sampled mid-step positions
+        want = a1 * I1 * np.exp(-a1 * zq) + a2 * I2 * np.exp(-a2 * zq)
+        assert Q.shape == (1, nq, g["ny"], g["nx"])
+        assert np.max(np.abs(Q[0] / want[:, None, None] - 1)) < 1e-12
+
+
+def test_heat_source_two_photon_term_closed_form():
+    A0, b1, b2 = 2e7, 3e-11, 5e-11
+    g, c, bm, A1 = plane_wave_case(A0, nz=400, d_eff=0.0, beta1=b1, beta2=b2)
+    dz = c["L"] / g["nz"]
+    o = oracle.Oracle(g, c, [bm])
+    Q = o.set_heat_output(8)
+    o.propagate(A1, 0.5 * A1)
+    I1 = EPS0 * C0 * c["n1"] * A0 ** 2 / 2
+    I2 = EPS0 * C0 * c["n2"] * (0.5 * A0) ** 2 / 2
+    # mean of the source before (I at z_n) and after (I at z_{n+1}) the nonlinear step
+    want = 0.0
+    for za in (np.array(q_steps(g["nz"], 8)) * dz, (np.array(q_steps(g["nz"], 8)) + 1.0) * dz):
+        want = want + 0.5 * (b1 * (I1 / (1 + b1 * I1 * za)) ** 2 + b2 * (I2 / (1 + b2 * I2 * za)) ** 2)
+    assert np.max(np.abs(Q[0] / want[:, None, None] - 1)) < 1e-9
+
+
+def test_heat_source_balances_the_power_the_fields_lose():
+    """Focused, converting beam with absorption and TPA: integral of q over the crystal = P(0) - P(L)."""
+    c = wl.crystal(20e-3, alpha=True, alpha1=2.0, alpha2=15.0, beta2=4e-11)
+    bm = wl.beam(c, 40.0, 1.2, 10.0)
+    n, nz = 64, 200
+    g = dict(nx=n, ny=n, nz=nz, nzt=0)
+    o = oracle.Oracle(g, c, [bm])
+    Q = o.set_heat_output(nz)
+    o.propagate(wl.gaussian_pump(n, n, c, bm).astype(np.complex128)[None])
+    h = o.power_history()
+    lost = h[0].sum() - h[-1].sum()
+    absorbed = Q.sum() * (bm["lx"] / n) * (bm["ly"] / n) * (c["L"] / nz)
+    assert lost / h[0].sum() > 0.05
+    assert abs(absorbed / lost - 1) < 2e-5                          # midpoint rule in z, O(dz^2)
+    # coarse sampling still integrates a smooth q
+    o2 = oracle.Oracle(g, c, [bm])
+    Q2 = o2.set_heat_output(25)
+    o2.propagate(wl.gaussian_pump(n, n, c, bm).astype(np.complex128)[None])
+    assert abs(Q2.sum() * (bm["lx"] / n) * (bm["ly"] / n) * (c["L"] / 25) / lost - 1) < 5e-3
