@@ -117,6 +117,15 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
 int shg_propagate_host(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out,
                        int batch, void* cuda_stream);
 
+/* Internal heat source of P:118 (Eq. 8), q = sum_j alpha_j I_j + beta_j I_j^2 with I_j = eps0 c n_j |A_j|^2 / 2
+ * (P:120), in W/m^3 -- the quantity the paper's thermal solver consumes (S§8(f) rank 1).  Q: DEVICE fp32
+ * [batch capacity][nq][ny][nx], 1 <= nq <= nz, BORROWED: every later shg_propagate fills it on its stream.
+ * Plane k holds the mean of q on the real-space fields right before and right after the nonlinear step of
+ * z-step n_k = floor((2k+1) nz / (2 nq)), i.e. q at z = z_{n_k} + dz/2 to second order in dz: the middle of
+ * the cell [k L/nq, (k+1) L/nq) rounded to a step (reading G27 of DESIGN.md).  Q == NULL switches it off.
+ * It is written from the epilogue of the nonlinear step: 2 extra sweeps over a row on nq of the nz steps. */
+int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq);
+
 /* Power (W) of both fields of `member` at the recorded node nearest to z (nodes z_n = n L/nz, n = 0..nz).
  * The SH efficiency is derived by the caller: eta = P2(L) / (P1(0) + P2(0))  (G16). */
 int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2);

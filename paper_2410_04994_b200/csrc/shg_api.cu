@@ -118,6 +118,9 @@ struct shg_ctx {
     double* d_hist = nullptr;
     unsigned int* d_barrier = nullptr;   // [0] barrier counter, [1] status word
     float* d_T_owned = nullptr;
+    float* d_Q = nullptr;              // borrowed heat-source output (shg_set_heat_output)
+    int nq = 0;
+    int* d_qmap = nullptr;             // [nz] z-step -> plane of Q, or -1
     size_t T_owned_bytes = 0;
     float2* d_stage[2] = {nullptr, nullptr};
     long long* d_trace = nullptr;
@@ -220,6 +223,11 @@ int upload_tables(shg_ctx* ctx) {
         m.Tpm_lo = (float)(c.T_pm - (double)m.Tpm_hi);
         m.dk0 = (float)c.dk0;
         m.dk_uniform = c.dk0 + c.ddk_dT * (ctx->T_uniform - c.T_pm);
+        {   // heat source per |A_j|^2 (Eq. 8 with I_j = c_j |A_j|^2, c_j = eps0 c n_j / 2)
+            const double c1 = 0.5 * EPS0 * C0 * nj[0], c2 = 0.5 * EPS0 * C0 * nj[1];
+            m.qa1 = (float)(alpha[0] * c1); m.qb1 = (float)(beta[0] * c1 * c1);
+            m.qa2 = (float)(alpha[1] * c2); m.qb2 = (float)(beta[1] * c2 * c2);
+        }
         const double dxdy = (bm.lx / g.nx) * (bm.ly / g.ny);
         for (int f = 0; f < 2; ++f) {
             m.pscale_in[f] = 0.5 * EPS0 * C0 * nj[f] * dxdy;
@@ -263,6 +271,7 @@ void free_ctx(shg_ctx* ctx) {
     cudaFree(ctx->d_hist);
     cudaFree(ctx->d_barrier);
     cudaFree(ctx->d_T_owned);
+    cudaFree(ctx->d_qmap);
     cudaFree(ctx->d_trace);
     for (int i = 0; i < 2; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -390,6 +399,7 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
     const size_t bytes = sizeof(float) * (size_t)(per_member ? ctx->g.batch : 1) * ctx->g.nzt * np_of(ctx);
     if (ctx->T_owned_bytes < bytes) {
         cudaFree(ctx->d_T_owned);
+    cudaFree(ctx->d_qmap);
         ctx->d_T_owned = nullptr;
         ctx->T_owned_bytes = 0;
         CU(cudaMalloc((void**)&ctx->d_T_owned, bytes));
@@ -397,6 +407,27 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
     }
     CU(cudaMemcpyAsync(ctx->d_T_owned, T_host, bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
     return shg_set_temperature(ctx, ctx->d_T_owned, T_uniform, per_member);
+}
+
+int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq) {
+    if (!ctx) return SHG_EINVAL;
+    if (!Q_device) { ctx->d_Q = nullptr; ctx->nq = 0; return SHG_OK; }
+    const int nz = ctx->g.nz;
+    if (nq < 1 || nq > nz || !aligned16(Q_device)) return SHG_EINVAL;
+    if (nq != ctx->nq || !ctx->d_qmap) {
+        std::vector<int> map((size_t)nz, -1);
+        for (int k = 0; k < nq; ++k) {
+            long long nk = ((2LL * k + 1) * nz) / (2LL * nq);
+            if (nk > nz - 1) nk = nz - 1;
+            map[(size_t)nk] = k;
+        }
+        CU(cudaStreamSynchronize(ctx->last_stream));      // an earlier propagate may still read the old map
+        if (!ctx->d_qmap) CU(cudaMalloc((void**)&ctx->d_qmap, sizeof(int) * (size_t)nz));
+        CU(cudaMemcpy(ctx->d_qmap, map.data(), sizeof(int) * (size_t)nz, cudaMemcpyHostToDevice));
+    }
+    ctx->d_Q = Q_device;
+    ctx->nq = nq;
+    return SHG_OK;
 }
 
 int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out, int batch,
@@ -424,6 +455,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     for (int hs = 0; hs < 2; ++hs) { P.hx[hs] = ctx->d_hx[hs]; P.hy[hs] = ctx->d_hy[hs]; }
     P.mem = ctx->d_mem;
     P.hist = ctx->d_hist;
+    P.Q = ctx->d_Q; P.qmap = ctx->d_qmap; P.nq = ctx->nq;
     P.barrier = ctx->d_barrier;
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
     P.trace = ctx->d_trace;

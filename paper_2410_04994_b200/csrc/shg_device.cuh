@@ -294,7 +294,8 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
 //   ROW_FINAL : A -> F_x -> conj -> A (output, real space)
 // smem_cta: base of the per-warp line regions.  hsel: 0 = full-step tables, 1 = half-step tables.
 // ------------------------------------------------------------------------------------------------
-template <int NX, int MODE, bool PREC>
+// HEAT: also write the heat source of Eq. 8 (a separate instantiation: the common path carries none of it).
+template <int NX, int MODE, bool PREC, bool HEAT = false>
 __device__ __forceinline__ void row_item(const Params& P, int item, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane) {
     using GE = Geo<NX>;
@@ -388,6 +389,24 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float2* p2 = (f ? own : par + M * H) + m;
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz, g1 = mb.g1dz, g2 = mb.g2dz;
         float s1 = 0.f, s2 = 0.f;
+        // Heat source of Eq. 8 for the plane that samples this z-step, if any (warp-uniform): half of
+        // q on the fields before the nonlinear step now, the other half after it (G27).  Only nq of the nz
+        // steps come here, so the two extra sweeps over the line in shared memory stay off the common path.
+        float* qrow = nullptr;
+        if constexpr (HEAT) {
+            const int kq = P.qmap[n];
+            if (kq >= 0) qrow = P.Q + (((size_t)b * P.nq + kq) * P.ny + y) * NX + rot + m;
+        }
+        auto heat_half = [&](bool first) {
+#pragma unroll 4
+            for (int q = 0; q < H; ++q) {
+                const float2 a1 = p1[M * q], a2 = p2[M * q];
+                const float i1 = fmaf(a1.x, a1.x, a1.y * a1.y), i2 = fmaf(a2.x, a2.x, a2.y * a2.y);
+                const float h = 0.5f * fmaf(i1, fmaf(mb.qb1, i1, mb.qa1), i2 * fmaf(mb.qb2, i2, mb.qa2));
+                if (first) qrow[M * q] = h; else qrow[M * q] += h;
+            }
+        };
+        if constexpr (HEAT) { if (qrow) heat_half(true); }
         if (P.nzt == 0) {
             // uniform temperature: phi(z) = dk z exactly; three sampled phases per step, warp-uniform
             const double TWO_PI = 6.283185307179586476925286766559;
@@ -447,6 +466,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                 point(q + 1, nxt);
             }
         }
+        if constexpr (HEAT) { if (qrow) heat_half(false); }
         s1 = warp_sum(s1); s2 = warp_sum(s2);
         if (lane == 0) {
             double* hst = P.hist + ((size_t)b * (P.nz + 1) + (n + 1)) * 2;
@@ -576,7 +596,7 @@ __device__ __forceinline__ const float4* load_twiddles(unsigned char* smem_raw, 
     return tws;
 }
 
-template <int NX, int MODE, bool PREC>
+template <int NX, int MODE, bool PREC, bool HEAT = false>
 __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane) {
     using GE = Geo<NX>;
@@ -586,7 +606,7 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
     if (slot >= P.row_slots) return;
     if (P.stagger_row > 0 && (slot & 1)) { const long long t0 = clock64(); while (clock64() - t0 < P.stagger_row) {} }
     for (int it = lo + slot; it < hi; it += P.row_slots)
-        row_item<NX, MODE, PREC>(P, it, n, hsel, smem_cta, tws, warp, lane);
+        row_item<NX, MODE, PREC, HEAT>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
 
 template <int NY, bool PREC, int NXC>
@@ -606,12 +626,12 @@ __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem
 // ------------------------------------------------------------------------------------------------
 // Per-pass kernels (two launches per z-step; any nx, ny)
 // ------------------------------------------------------------------------------------------------
-template <int NX, int MODE, bool PREC>
+template <int NX, int MODE, bool PREC, bool HEAT = false>
 __global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row(Params P, int n, int hsel) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
-    row_pass<NX, MODE, PREC>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
+    row_pass<NX, MODE, PREC, HEAT>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 template <int NY, bool PREC>
@@ -679,7 +699,7 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
     return ok != 0;
 }
 
-template <int N, bool PREC>
+template <int N, bool PREC, bool HEAT = false>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -689,7 +709,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        row_pass<N, ROW_MID, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
+        row_pass<N, ROW_MID, PREC, HEAT>(P, n, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;

@@ -18,11 +18,11 @@ cudaError_t set_smem(K kernel, int bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
-template <int MODE, bool PREC>
+template <int MODE, bool PREC, bool HEAT = false>
 cudaError_t launch_row_t(const Params& P, int n, int hsel, int grid, cudaStream_t st) {
-    cudaError_t e = set_smem(k_row<N, MODE, PREC>, GE::CTA_SMEM);
+    cudaError_t e = set_smem(k_row<N, MODE, PREC, HEAT>, GE::CTA_SMEM);
     if (e != cudaSuccess) return e;
-    k_row<N, MODE, PREC><<<grid, GE::THREADS, GE::CTA_SMEM, st>>>(P, n, hsel);
+    k_row<N, MODE, PREC, HEAT><<<grid, GE::THREADS, GE::CTA_SMEM, st>>>(P, n, hsel);
     return cudaGetLastError();
 }
 
@@ -34,18 +34,18 @@ cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-template <bool PREC>
+template <bool PREC, bool HEAT>
 cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
     const int smem = GE::CTA_SMEM;
-    cudaError_t e = set_smem(k_persist<N, PREC>, smem);
+    cudaError_t e = set_smem(k_persist<N, PREC, HEAT>, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persist<N, PREC>, GE::THREADS, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persist<N, PREC, HEAT>, GE::THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     Params Pc = P;
     void* args[] = {&Pc};
-    return cudaLaunchCooperativeKernel((const void*)k_persist<N, PREC>, dim3(grid), dim3(GE::THREADS), args,
+    return cudaLaunchCooperativeKernel((const void*)k_persist<N, PREC, HEAT>, dim3(grid), dim3(GE::THREADS), args,
                                        (size_t)smem, st);
 }
 }  // namespace
@@ -57,11 +57,13 @@ cudaError_t SHG_CAT(launch_row_, SHG_N)(const Params& P, int mode, int n, int hs
                                         cudaStream_t st) {
     if (prec) {
         if (mode == ROW_FIRST) return launch_row_t<ROW_FIRST, true>(P, n, hsel, grid, st);
-        if (mode == ROW_MID) return launch_row_t<ROW_MID, true>(P, n, hsel, grid, st);
+        if (mode == ROW_MID) return P.Q ? launch_row_t<ROW_MID, true, true>(P, n, hsel, grid, st)
+                                        : launch_row_t<ROW_MID, true>(P, n, hsel, grid, st);
         return launch_row_t<ROW_FINAL, true>(P, n, hsel, grid, st);
     } else {
         if (mode == ROW_FIRST) return launch_row_t<ROW_FIRST, false>(P, n, hsel, grid, st);
-        if (mode == ROW_MID) return launch_row_t<ROW_MID, false>(P, n, hsel, grid, st);
+        if (mode == ROW_MID) return P.Q ? launch_row_t<ROW_MID, false, true>(P, n, hsel, grid, st)
+                                        : launch_row_t<ROW_MID, false>(P, n, hsel, grid, st);
         return launch_row_t<ROW_FINAL, false>(P, n, hsel, grid, st);
     }
 }
@@ -71,7 +73,8 @@ cudaError_t SHG_CAT(launch_col_, SHG_N)(const Params& P, int hsel, bool prec, in
 }
 
 cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid, cudaStream_t st) {
-    return prec ? launch_persist_t<true>(P, grid, st) : launch_persist_t<false>(P, grid, st);
+    if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
+    return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
 }
 
 LaunchInfo SHG_CAT(launch_info_, SHG_N)() {

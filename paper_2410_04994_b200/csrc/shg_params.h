@@ -16,6 +16,7 @@ struct MemberDev {
     float dk0;
     double dk_uniform;         // dk0 + ddk_dT (T_uniform - T_pm), used when nzt == 0
     double dzd;
+    float qa1, qb1, qa2, qb2;  // heat source of Eq. 8 per |A_j|^2: q = s1 (qa1 + qb1 s1) + s2 (qa2 + qb2 s2), s_j = |A_j|^2
     double pscale_in[2];       // (eps0 c n_j/2) dx dy
     double pscale_step[2];     // exp(-alpha_j dz/2) (eps0 c n_j/2) dx dy  (Parseval: power after the closing half-step)
 };
@@ -36,6 +37,9 @@ struct Params {
     const float4* hy[2];       // [batch][2][ny], includes 1/(nx ny)
     const MemberDev* mem;      // [batch]
     double* hist;              // [batch][nz+1][2]
+    float* Q;                  // optional heat-source output [batch][nq][ny][nx] (shg_set_heat_output), else null
+    const int* qmap;           // [nz]: plane of Q that samples z-step n, or -1
+    int nq;
     unsigned int* barrier;     // grid barrier counter (persistent kernel)
     int* status;               // device status word (barrier timeout)
     long long* trace;          // optional phase timeline of the persistent kernel (SHG_OPT_TRACE), else null:

@@ -18,7 +18,7 @@ SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
 OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE = 1, 2, 3, 4
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
-           "shg_propagate_host", "shg_power", "shg_power_history", "shg_gaussian_input",
+           "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
            "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak", "shg_last_launch_count", "shg_destroy", "shg_strerror")
 
 
@@ -68,6 +68,7 @@ def lib():
     L.shg_last_main_loop_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.shg_read_trace.argtypes = [vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.shg_last_launch_count.argtypes = [vp]
+    L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
     L.shg_measure_fp32_peak.argtypes = [dp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
@@ -187,6 +188,19 @@ class Shg:
                                    _dev_ptr(A1_out, ("complex64",)), _dev_ptr(A2_out, ("complex64",)),
                                    batch, _stream_ptr(stream)))
         return A1_out, A2_out
+
+    # -- shg_set_heat_output: Q is a CUDA float32 tensor [batch][nq][ny][nx] (kept alive here), None = off
+    def set_heat_output(self, Q=None):
+        g = self.grid
+        if Q is None:
+            self._Q = None
+            _check(lib().shg_set_heat_output(self._h, None, 0))
+            return self
+        if Q.dim() != 4 or Q.shape[0] != g["batch"] or Q.shape[2] != g["ny"] or Q.shape[3] != g["nx"]:
+            raise ValueError("Q must be [batch][nq][ny][nx]")
+        self._Q = Q
+        _check(lib().shg_set_heat_output(self._h, _dev_ptr(Q, ("float32",)), int(Q.shape[1])))
+        return self
 
     # -- shg_propagate_host: numpy complex64 arrays or (pinned) CPU tensors
     def propagate_host(self, A1_in, A2_in=None, A1_out=None, A2_out=None, stream=None):

@@ -336,3 +336,60 @@ def test_linear_path_has_no_power_drift_over_many_steps():
     torch.cuda.synchronize()
     h = ctx.power_history(0)
     assert np.max(np.abs(h[:, 0] / h[0, 0] - 1)) <= 2e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# heat source of Eq. 8, S§8(f) rank 1
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,nz,nq", [("cfg2", 60, 60), ("cfg2", 61, 7), ("cfg3", 24, 5), ("cfg5", 12, 3)])
+def test_heat_source_matches_oracle(name, nz, nq):
+    w = wl.make(name, nz=nz)
+    g = dict(w["grid"])
+    # reference run without the heat output: switching it on must not change the fields
+    r1, r2, _, _ = run_gpu(w)
+    ctx = shg.Shg(g, w["crystal"], w["beams"])
+    ctx.set_temperature(torch.from_numpy(w["T"]).cuda(), per_member=w["per_member"])
+    Q = torch.full((g["batch"], nq, g["ny"], g["nx"]), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.set_heat_output(Q)
+    g1, g2 = ctx.propagate(torch.from_numpy(w["A1"]).cuda())
+    torch.cuda.synchronize()
+    assert np.array_equal(g1.cpu().numpy(), r1) and np.array_equal(g2.cpu().numpy(), r2)
+    o = oracle.Oracle(g, w["crystal"], w["beams"])
+    o.set_temperature(w["T"], w["T_uniform"], w["per_member"])
+    Qo = o.set_heat_output(nq)
+    o.propagate(w["A1"].astype(np.complex128))
+    Qg = Q.cpu().numpy().astype(np.float64)
+    assert np.isfinite(Qg).all()                                   # every point of every plane was written
+    for k in range(nq):
+        err = np.linalg.norm((Qg[0, k] - Qo[0, k]).ravel()) / np.linalg.norm(Qo[0, k].ravel())
+        assert err <= TOL_FIELD, "plane %d rel-L2 %.3e" % (k, err)
+    # and the next propagate without it leaves the array alone
+    ctx.set_heat_output(None)
+    Q.fill_(-1.0)
+    ctx.propagate(torch.from_numpy(w["A1"]).cuda())
+    torch.cuda.synchronize()
+    assert float(Q.max()) == -1.0
+
+
+def test_heat_source_batch_and_per_pass_launches():
+    """Batched members with their own windows (cfg4-like), uniform T, per-pass launch scheme; argument errors."""
+    w = wl.make("cfg4", nz=16)
+    g = dict(w["grid"], batch=6)
+    beams = [w["beams"][b] for b in (0, 9, 18, 27, 36, 63)]
+    A1 = np.stack([w["A1"][b] for b in (0, 9, 18, 27, 36, 63)])
+    for persistent in (True, False):
+        ctx = shg.Shg(g, w["crystal"], beams, persistent=persistent)
+        ctx.set_temperature(None, w["T_uniform"])
+        Q = torch.zeros((6, 4, g["ny"], g["nx"]), dtype=torch.float32, device="cuda")
+        ctx.set_heat_output(Q)
+        ctx.propagate(torch.from_numpy(A1).cuda())
+        torch.cuda.synchronize()
+        o = oracle.Oracle(g, w["crystal"], beams)
+        o.set_temperature(None, w["T_uniform"], False)
+        Qo = o.set_heat_output(4)
+        o.propagate(A1.astype(np.complex128))
+        Qg = Q.cpu().numpy().astype(np.float64)
+        for b in range(6):
+            assert np.linalg.norm((Qg[b] - Qo[b]).ravel()) / np.linalg.norm(Qo[b].ravel()) <= TOL_FIELD
+    with pytest.raises(shg.ShgError):
+        ctx.set_heat_output(torch.zeros((6, 17, g["ny"], g["nx"]), dtype=torch.float32, device="cuda"))   # nq > nz
