@@ -35,7 +35,8 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", help="cfg2 | cfg3 | cfg4 | cfg5 (default: the largest single-GPU config)")
+    ap.add_argument("--workload", default="cfg5", help="cfg2 | cfg3 | cfg4 | cfg5 (default: the largest single-GPU config) | stream256 | stream1024 "
+                         "(sweeps whose field state is larger than L2)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--nz", type=int, default=None, help="override the z-step count (profiling runs only; "
                     "a number measured with --nz is not the config's)")
@@ -217,7 +218,9 @@ def workload_label(w):
               "cfg2": "BASELINE.json configs[1]: 128x128, 1000 z-steps, absorption + T array",
               "cfg3": "BASELINE.json configs[2]: 256x256, 4000 z-steps, T array",
               "cfg4": "BASELINE.json configs[3]: 64 x (128x128, 1000 z-steps) parameter sweep",
-              "cfg5": "BASELINE.json configs[4]: 1024x1024, 10000 z-steps, 1 GiB T array"}
+              "cfg5": "BASELINE.json configs[4]: 1024x1024, 10000 z-steps, 1 GiB T array",
+              "stream256": "throughput regime (SURVEY 8(f) rank 3): 192 x (256x256), 201 MB of fields > L2",
+              "stream1024": "throughput regime (SURVEY 8(f) rank 3): 16 x (1024x1024), 268 MB of fields > L2"}
     return labels.get(w["name"], w["name"])
 
 

@@ -61,6 +61,8 @@ typedef struct {
     double dk0, ddk_dT, T_pm;           /* rad/m, rad/(m K), same unit as T                           */
     double alpha1, alpha2;              /* linear intensity absorption, 1/m                           */
     double beta1, beta2;                /* two-photon absorption, m/W                                 */
+    double rho1, rho2;                  /* spatial walk-off angles along x, rad: term tan(rho) dA/dx of P:387
+                                           (the paper's runs use 0; P:314 names it for birefringent crystals) */
 } shg_crystal;
 
 /* One batch member's beam and transverse window (Eq. 5-6). */
@@ -87,6 +89,8 @@ typedef struct {
                                   with L2-only loads (ld.global.cg) and no fence is issued; 1: additionally issue a
                                   gpu-scope acquire fence (invalidates L1) after every barrier, as the letter of
                                   the PTX memory model asks.  Bit-identical results; ~350 SM clocks per barrier.   */
+#define SHG_OPT_UNDEPLETED 5    /* 1: drop the coupling term of dA1/dz (the pump only diffracts and is absorbed), the
+                                  "dPump = 0" check against Boyd-Kleinman of P:292; 0 (default): full Eq. 2.       */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);

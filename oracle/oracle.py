@@ -27,7 +27,7 @@ class Grid(C.Structure):
 
 class Crystal(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("L", "lambda1", "n1", "n2", "d_eff", "dk0", "ddk_dT", "T_pm",
-                                          "alpha1", "alpha2", "beta1", "beta2")]
+                                          "alpha1", "alpha2", "beta1", "beta2", "rho1", "rho2")]
 
 
 class Beam(C.Structure):

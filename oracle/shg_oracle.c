@@ -278,8 +278,6 @@ static inline void rk4_point(const nl_par* p, cplx* A1, cplx* A2, double h,
     *A2 += (h / 6.0) * (k1b + 2.0 * k2b + 2.0 * k3b + k4b);
 }
 
-/* Factor of the linear step of length h for one field (P:143 L_j; P:346-352 Eq. A.4-A.5; sign G3):
- *   Hj[my][mx] = exp(-i (kx^2+ky^2) h / (2 k_j) - alpha_j h / 2),  kx = 2 pi m'/lx, m' = m or m-nx (G11) */
 /* q = sum_j alpha_j I_j + beta_j I_j^2,  I_j = eps0 c n_j |A_j|^2 / 2   (Eq. 8) */
 static inline double heat_source(const nl_par* p, const orc_crystal* c, cplx A1, cplx A2) {
     double I1 = p->c1 * (creal(A1) * creal(A1) + cimag(A1) * cimag(A1));
@@ -287,7 +285,12 @@ static inline double heat_source(const nl_par* p, const orc_crystal* c, cplx A1,
     return c->alpha1 * I1 + c->beta1 * I1 * I1 + c->alpha2 * I2 + c->beta2 * I2 * I2;
 }
 
-static cplx* linear_factor(const orc_grid* g, const orc_beam* bm, double kj, double alpha, double h) {
+/* Factor of the linear step of length h for one field (P:143 L_j; P:346-352 Eq. A.4-A.5; sign G3):
+ *   Hj[my][mx] = exp(-i (kx^2+ky^2) h / (2 k_j) - i kx tan(rho_j) h - alpha_j h / 2),  kx = 2 pi m'/lx,
+ *   m' = m or m-nx (G11).
+ * The walk-off term tan(rho) dA/dx of P:387 (G21): the field of a beam with walk-off angle rho moves by
+ * +tan(rho) h along x.                                                                              */
+static cplx* linear_factor(const orc_grid* g, const orc_beam* bm, double kj, double alpha, double rho, double h) {
     int nx = g->nx, ny = g->ny;
     cplx* H = (cplx*)malloc(sizeof(cplx) * (size_t)nx * ny);
     for (int my = 0; my < ny; ++my) {
@@ -296,7 +299,7 @@ static cplx* linear_factor(const orc_grid* g, const orc_beam* bm, double kj, dou
         for (int mx = 0; mx < nx; ++mx) {
             int sx = (mx < nx / 2) ? mx : mx - nx;
             double kx = 2.0 * ORC_PI * (double)sx / bm->lx;
-            double ang = -(kx * kx + ky * ky) * h / (2.0 * kj);
+            double ang = -(kx * kx + ky * ky) * h / (2.0 * kj) - kx * tan(rho) * h;
             H[(size_t)my * nx + mx] = exp(-0.5 * alpha * h) * (cos(ang) + I * sin(ang));
         }
     }
@@ -357,8 +360,8 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
 
     /* linear factors: half step for scheme 0, full step for scheme 1 */
     const double hlin = (ctx->o.scheme == 0) ? 0.5 * dz : dz;
-    cplx* H1 = linear_factor(g, bm, k1, c->alpha1, hlin);
-    cplx* H2 = linear_factor(g, bm, k2, c->alpha2, hlin);
+    cplx* H1 = linear_factor(g, bm, k1, c->alpha1, c->rho1, hlin);
+    cplx* H2 = linear_factor(g, bm, k2, c->alpha2, c->rho2, hlin);
 
     double* phi  = (double*)calloc(np, sizeof(double));
     double* Tcur = (double*)malloc(sizeof(double) * np);

@@ -48,6 +48,7 @@ typedef struct {
     double dk0, ddk_dT, T_pm;      /* dk(T) = dk0 + ddk_dT (T - T_pm)   [rad/m, rad/(m K), K or C]   */
     double alpha1, alpha2;         /* linear intensity absorption, 1/m                               */
     double beta1, beta2;           /* two-photon absorption, m/W (G5)                                */
+    double rho1, rho2;             /* spatial walk-off angles along x, rad (0 in the paper's runs) */
 } orc_crystal;
 
 /* Per-member beam / window.  P:95-104 (Eq. 5-6). P, w0, focus_z are used only by orc_gaussian_input. */

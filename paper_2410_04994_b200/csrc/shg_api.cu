@@ -103,6 +103,7 @@ struct shg_ctx {
     bool persistent = true;
     bool precise = true;
     bool acquire_fence = false;
+    bool undepleted = false;
     bool tables_dirty = true;
 
     Launchers Lx{}, Ly{};
@@ -159,6 +160,7 @@ int upload_tables(shg_ctx* ctx) {
     const double alpha[2] = {c.alpha1, c.alpha2};
     const double beta[2] = {c.beta1, c.beta2};
     const double nj[2] = {c.n1, c.n2};
+    const double tanrho[2] = {std::tan(c.rho1), std::tan(c.rho2)};
     const bool prec = ctx->precise;
     auto mk = [&](double re, double im) {
         float4 w = split4(re, im);
@@ -194,7 +196,8 @@ int upload_tables(shg_ctx* ctx) {
                     for (int m = 0; m < n; ++m) {
                         const int ms = (m < n / 2) ? m : m - n;
                         const double kk = 2.0 * PI * (double)ms / len;
-                        const double ang = -kk * kk * h / (2.0 * k[f]);
+                        // diffraction; along x also the walk-off term tan(rho) dA/dx of P:387 (G21)
+                        const double ang = -kk * kk * h / (2.0 * k[f]) - (axis ? 0.0 : kk * tanrho[f] * h);
                         const double mag = std::exp(-0.25 * alpha[f] * h) * scale;
                         tab[((size_t)b * 2 + f) * n + m] = mk(mag * std::cos(ang), mag * std::sin(ang));
                     }
@@ -212,7 +215,7 @@ int upload_tables(shg_ctx* ctx) {
     for (int b = 0; b < B; ++b) {
         shg::MemberDev& m = mem[b];
         const shg_beam& bm = ctx->beams[b];
-        m.kap1dz = (float)(kappa1 * dz);
+        m.kap1dz = ctx->undepleted ? 0.f : (float)(kappa1 * dz);     // undepleted pump
         m.kap2dz = (float)(kappa2 * dz);
         m.g1dz = (float)(0.5 * beta[0] * 0.5 * EPS0 * C0 * nj[0] * dz);
         m.g2dz = (float)(0.5 * beta[1] * 0.5 * EPS0 * C0 * nj[1] * dz);
@@ -355,6 +358,9 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
     switch (option) {
         case SHG_OPT_PERSISTENT: ctx->persistent = (value != 0); return SHG_OK;
         case SHG_OPT_ACQUIRE_FENCE: ctx->acquire_fence = (value != 0); return SHG_OK;
+        case SHG_OPT_UNDEPLETED:
+            if (ctx->undepleted != (value != 0)) { ctx->undepleted = (value != 0); ctx->tables_dirty = true; }
+            return SHG_OK;
         case SHG_OPT_PRECISE:
             if (ctx->precise != (value != 0)) { ctx->precise = (value != 0); ctx->tables_dirty = true; }
             return SHG_OK;

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libshg.so")
 
 SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
-OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE = 1, 2, 3, 4
+OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE, OPT_UNDEPLETED = 1, 2, 3, 4, 5
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
@@ -29,7 +29,7 @@ class Grid(C.Structure):
 
 class Crystal(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("L", "lambda1", "n1", "n2", "d_eff", "dk0", "ddk_dT", "T_pm",
-                                          "alpha1", "alpha2", "beta1", "beta2")]
+                                          "alpha1", "alpha2", "beta1", "beta2", "rho1", "rho2")]
 
 
 class Beam(C.Structure):

@@ -21,6 +21,7 @@ C0 = 299792458.0
 T_PM = 56.5   # oven temperature quoted at PAPER.md:292; only T - T_pm enters the model
 
 CONFIG_NAMES = ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5")
+STREAM_NAMES = ("stream256", "stream1024")   # working set larger than L2
 
 
 def crystal(L, alpha=False, ddk_dT=0.0, **over):
@@ -153,6 +154,17 @@ def make(name: str, nz: int | None = None, batch: int | None = None):
         beams = [bm]
         nzt = 256
         T = _bump_field(nx, ny, nzt, c, bm, seed=5)
+    elif name in ("stream256", "stream1024"):
+        # Throughput regime: a sweep whose field state (16 B/pt) is larger than the
+        # 126 MB L2, so every pass really streams through HBM.  Members: pump power log-spaced over 1-100 W at
+        # xi = 2.84 in the cfg2 / cfg5 crystal, uniform T_pm + 0.5 K (as cfg4), each on its own window.
+        nx = ny = 256 if name == "stream256" else 1024
+        members = (192 if nx == 256 else 16) if batch is None else batch       # 201 MB / 268 MB of fields
+        nzs = 200 if nz is None else nz
+        c = crystal(30e-3 if nx == 256 else 40e-3, alpha=True, ddk_dT=-30.0)
+        beams = [beam(c, float(P), 2.84, 8.0 if nx == 256 else 10.0) for P in np.geomspace(1.0, 100.0, members)]
+        nzt = 0
+        T_uniform = T_PM + 0.5
     else:
         raise ValueError("unknown workload %r" % name)
     grid = dict(nx=nx, ny=ny, nz=nzs, nzt=nzt, batch=len(beams))

@@ -393,3 +393,51 @@ def test_heat_source_batch_and_per_pass_launches():
             assert np.linalg.norm((Qg[b] - Qo[b]).ravel()) / np.linalg.norm(Qo[b].ravel()) <= TOL_FIELD
     with pytest.raises(shg.ShgError):
         ctx.set_heat_output(torch.zeros((6, 17, g["ny"], g["nx"]), dtype=torch.float32, device="cuda"))   # nq > nz
+
+
+@pytest.mark.parametrize("name", ["stream256", "stream1024"])
+def test_stream_workloads_reduced_batch_against_oracle(name):
+    """The throughput-regime sweeps (fields larger than L2) at a batch and length the oracle can follow."""
+    w = wl.make(name, nz=10, batch=3)
+    g1, g2, gh, _ = run_gpu(w)
+    o1, o2, oh = run_oracle(w)
+    check(w, g1, g2, gh, o1, o2, oh, tol_field=2e-5, tol_eta=2e-5)
+
+
+def test_undepleted_pump_option_matches_oracle_switch():
+    """SHG_OPT_UNDEPLETED (the paper's Boyd-Kleinman check) against the oracle's own switch."""
+    w = wl.make("cfg1", nz=60)
+    g = dict(w["grid"])
+    ctx = shg.Shg(g, w["crystal"], w["beams"])
+    ctx.set_option(shg.OPT_UNDEPLETED, 1)
+    ctx.set_temperature(None, w["T_uniform"])
+    g1, g2 = ctx.propagate(torch.from_numpy(w["A1"]).cuda())
+    torch.cuda.synchronize()
+    gh = ctx.power_history(0)
+    o = oracle.Oracle(g, w["crystal"], w["beams"], undepleted=True)
+    o.set_temperature(None, w["T_uniform"], False)
+    o1, o2 = o.propagate(w["A1"].astype(np.complex128))
+    oh = o.power_history(0)
+    assert rel_l2(g1.cpu().numpy(), o1) <= 2e-5 and rel_l2(g2.cpu().numpy(), o2) <= 2e-5
+    assert abs(gh[-1, 1] / oh[-1, 1] - 1) <= 2e-5
+    assert abs(gh[-1, 0] / gh[0, 0] - 1) <= 1e-6                      # the pump is not depleted
+    ctx.set_option(shg.OPT_UNDEPLETED, 0)                             # and the option can be switched back
+    d1, d2 = ctx.propagate(torch.from_numpy(w["A1"]).cuda())
+    torch.cuda.synchronize()
+    assert ctx.power_history(0)[-1, 0] / gh[0, 0] < 0.95
+
+
+def test_walk_off_matches_oracle():
+    """Walk-off angles on both fields, full coupled run on an asymmetric input."""
+    c = wl.crystal(10e-3, alpha=True, ddk_dT=-30.0, rho1=-1.0e-3, rho2=2.5e-3)
+    bm = wl.beam(c, 20.0, 1.5, 8.0)
+    n, nz = 128, 40
+    g = dict(nx=n, ny=n, nz=nz, nzt=0, batch=1)
+    A1 = np.roll(wl.gaussian_pump(n, n, c, bm), (5, -3), axis=(0, 1))[None]
+    w = dict(name="walkoff", grid=g, crystal=c, beams=[bm], T=None, T_uniform=wl.T_PM + 0.3, per_member=False, A1=A1)
+    g1, g2, gh, _ = run_gpu(w)
+    o1, o2, oh = run_oracle(w)
+    check(w, g1, g2, gh, o1, o2, oh, tol_field=2e-5, tol_eta=2e-5)
+    w0 = dict(w, crystal=dict(c, rho1=0.0, rho2=0.0))
+    z1, z2, _, _ = run_gpu(w0)
+    assert rel_l2(g2, z2) > 1e-2                                      # the angles matter at this size

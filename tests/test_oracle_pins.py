@@ -491,3 +491,34 @@ def test_heat_source_balances_the_power_the_fields_lose():
     Q2 = o2.set_heat_output(25)
     o2.propagate(wl.gaussian_pump(n, n, c, bm).astype(np.complex128)[None])
     assert abs(Q2.sum() * (bm["lx"] / n) * (bm["ly"] / n) * (c["L"] / 25) / lost - 1) < 5e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# 14. spatial walk-off ("tan(rho) dA/dx"; G21): a pure translation by tan(rho) z along x
+# ------------------------------------------------------------------------------------------------
+def test_walk_off_translates_the_beam_along_x_only():
+    c = wl.crystal(20e-3, d_eff=0.0, rho1=0.0, rho2=4e-3)
+    bm = wl.beam(c, 1.0, 1.0, 16.0)
+    n, nz = 128, 8
+    dx = bm["lx"] / n
+    # choose rho so that the total shift is a whole number of grid cells: the periodic shift is then exact
+    cells = 5
+    c["rho2"] = math.atan(cells * dx / c["L"])
+    c["rho1"] = math.atan(-2 * dx / c["L"])
+    A = wl.gaussian_pump(n, n, c, bm).astype(np.complex128)
+    Ain2 = np.roll(A, 7, axis=0) * (0.3 + 0.1j)                    # off-centre in y: a shift in y would show
+    ref = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=0), dict(c, rho1=0.0, rho2=0.0), [bm])
+    r1, r2 = ref.propagate(A[None], Ain2[None])
+    o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=0), c, [bm])
+    o1, o2 = o.propagate(A[None], Ain2[None])
+    s1 = np.linalg.norm(r1)
+    assert np.linalg.norm(o2[0] - np.roll(r2[0], cells, axis=1)) / np.linalg.norm(r2) < 1e-11   # SH: +5 cells in x
+    assert np.linalg.norm(o1[0] - np.roll(r1[0], -2, axis=1)) / s1 < 1e-11                      # FH: -2 cells
+    assert np.linalg.norm(o2[0] - r2[0]) / np.linalg.norm(r2) > 0.1                             # and it did move
+    # centroid of a non-integer shift: <x> moves by tan(rho) L
+    c2 = dict(c, rho1=1.3e-3, rho2=0.0)
+    o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=0), c2, [bm])
+    q1, _ = o.propagate(A[None])
+    x, _y = wl.axes(n, n, bm)
+    cen = lambda a: float((np.abs(a) ** 2 * x[None, :]).sum() / (np.abs(a) ** 2).sum())
+    assert abs((cen(q1[0]) - cen(r1[0])) / (math.tan(1.3e-3) * c["L"]) - 1) < 1e-9
