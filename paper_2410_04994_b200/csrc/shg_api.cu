@@ -127,8 +127,6 @@ struct shg_ctx {
     long long* d_trace = nullptr;
     int trace_steps = 0;        // steps recorded per propagate (0 = tracing off)
     int trace_grid = 0;         // CTAs of the last traced launch
-    int stagger_row = 0, stagger_col = 0;
-    int grid_cap = 0;           // experimental: cap on the number of CTAs (0 = one per SM)
 
     const float* d_T = nullptr;
     double T_uniform = 0.0;
@@ -364,9 +362,6 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
         case SHG_OPT_PRECISE:
             if (ctx->precise != (value != 0)) { ctx->precise = (value != 0); ctx->tables_dirty = true; }
             return SHG_OK;
-        case 100: ctx->stagger_row = value; return SHG_OK;
-        case 101: ctx->stagger_col = value; return SHG_OK;
-        case 102: ctx->grid_cap = value; return SHG_OK;
         case SHG_OPT_TRACE: {
             if (value < 0 || value > 4096) return SHG_EINVAL;
             if (value != ctx->trace_steps) {
@@ -465,7 +460,6 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.barrier = ctx->d_barrier;
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
     P.trace = ctx->d_trace;
-    P.stagger_row = ctx->stagger_row; P.stagger_col = ctx->stagger_col;
     P.acquire_fence = ctx->acquire_fence ? 1 : 0;
     P.trace_steps = ctx->trace_steps;
 
@@ -477,7 +471,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const shg::LaunchInfo ix = ctx->Lx.info(), iy = ctx->Ly.info();
     const int UR = batch * g.ny / ix.rows_per_item;          // row-pass items
     const int UC = batch * 2 * (g.nx / iy.cols_per_item);    // column-pass strips
-    const int max_grid = (ctx->grid_cap > 0 && ctx->grid_cap < ctx->sm_count) ? ctx->grid_cap : ctx->sm_count;
+    const int max_grid = ctx->sm_count;
     const int grid_r = UR < max_grid ? UR : max_grid;
     const int grid_c = UC < max_grid ? UC : max_grid;
     const bool use_persist = ctx->persistent && g.nx == g.ny;

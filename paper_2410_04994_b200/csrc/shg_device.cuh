@@ -80,7 +80,10 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads) {
 // Table loads whose address carries a (numerically void) dependency on an earlier result.  Without it ptxas
 // hoists all R twiddle / propagator loads (4 registers each) far above their use and spills the line data
 // to make room; chaining load k to product k - TABLE_DEPTH keeps TABLE_DEPTH loads in flight.  One LOP3 each.
-constexpr int TABLE_DEPTH = 6;
+// Measured on cfg5 (us per z-step): depth 4: 40.2, 6: 39.0, 8: 39.1, 12: 36.6, 16: 36.7, 20: 38.7, 31 (no chain): 40.7
+// (spills return); the propagator tables are the sensitive ones (twiddles 6..16 with tables at 12-14: 36.6-37.8).
+constexpr int TABLE_DEPTH = 12;      // global propagator tables (L1 latency)
+constexpr int TWIDDLE_DEPTH = 12;    // shared-memory twiddles
 
 template <int BYTE_OFF>
 __device__ __forceinline__ float4 lds128_after(unsigned saddr, float dep) {
@@ -128,7 +131,7 @@ __device__ __forceinline__ void table_mul(float2 (&v)[R], const float4* __restri
 template <int N, bool PREC, int K1>
 __device__ __forceinline__ void twiddle_one(float2 (&v)[FftCfg<N>::R], unsigned tws_saddr) {
     constexpr int M = FftCfg<N>::M;
-    const float dep = (K1 > TABLE_DEPTH) ? v[K1 - TABLE_DEPTH].x : v[K1].x;
+    const float dep = (K1 > TWIDDLE_DEPTH) ? v[K1 - TWIDDLE_DEPTH].x : v[K1].x;
     v[K1] = cmul_hl<false, PREC>(v[K1], lds128_after<K1 * M * 16>(tws_saddr, dep));
 }
 
@@ -604,7 +607,6 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
     cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
     if (slot >= P.row_slots) return;
-    if (P.stagger_row > 0 && (slot & 1)) { const long long t0 = clock64(); while (clock64() - t0 < P.stagger_row) {} }
     for (int it = lo + slot; it < hi; it += P.row_slots)
         row_item<NX, MODE, PREC, HEAT>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
@@ -618,7 +620,6 @@ __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem
     const int team = warp / GE::TW, trank = warp % GE::TW;
     float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
     if (team >= P.col_teams) return;
-    if (P.stagger_col > 0 && (team & 1)) { const long long t0 = clock64(); while (clock64() - t0 < P.stagger_col) {} }
     for (int it = lo + team; it < hi; it += P.col_teams)
         col_item<NY, PREC, NXC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
 }

@@ -23,7 +23,6 @@ struct MemberDev {
 
 struct Params {
     int nx, ny, nz, nzt, batch;
-    int stagger_row, stagger_col;  // experimental: start delay (SM clocks) of odd slots / teams
     int acquire_fence;         // 1: gpu-scope acquire fence after every device-wide barrier (SHG_OPT_ACQUIRE_FENCE)
     int row_slots, col_teams;  // slots (warps / warp pairs) and teams per CTA that take items (<= Geo limits)
     float2* A[2];              // working / output fields [batch][ny][nx]
