@@ -91,6 +91,11 @@ typedef struct {
                                   the PTX memory model asks.  Bit-identical results; ~350 SM clocks per barrier.   */
 #define SHG_OPT_UNDEPLETED 5    /* 1: drop the coupling term of dA1/dz (the pump only diffracts and is absorbed), the
                                   "dPump = 0" check against Boyd-Kleinman of P:292; 0 (default): full Eq. 2.       */
+#define SHG_OPT_SCHEME     6    /* 0 (default): L/2 - N(dz) - L/2 with neighbouring half-steps merged (north_star);
+                                  1: the paper's own ordering N(dz/2) - L(dz) - N(dz/2), Eq. 14-15:
+                                  two RK4 half-steps per z-step, powers summed at the true nodes.  Variant for
+                                  comparison with the paper's scheme (differs from scheme 0 by O(dz^2)); needs
+                                  SHG_OPT_PRECISE = 1 and no heat output (else shg_propagate returns SHG_EINVAL). */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);

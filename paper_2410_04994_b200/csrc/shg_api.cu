@@ -104,6 +104,7 @@ struct shg_ctx {
     bool precise = true;
     bool acquire_fence = false;
     bool undepleted = false;
+    int scheme = 0;
     bool tables_dirty = true;
 
     Launchers Lx{}, Ly{};
@@ -356,6 +357,10 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
     switch (option) {
         case SHG_OPT_PERSISTENT: ctx->persistent = (value != 0); return SHG_OK;
         case SHG_OPT_ACQUIRE_FENCE: ctx->acquire_fence = (value != 0); return SHG_OK;
+        case SHG_OPT_SCHEME:
+            if (value != 0 && value != 1) return SHG_EINVAL;
+            ctx->scheme = value;
+            return SHG_OK;
         case SHG_OPT_UNDEPLETED:
             if (ctx->undepleted != (value != 0)) { ctx->undepleted = (value != 0); ctx->tables_dirty = true; }
             return SHG_OK;
@@ -461,6 +466,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
     P.trace = ctx->d_trace;
     P.acquire_fence = ctx->acquire_fence ? 1 : 0;
+    P.scheme = ctx->scheme;
     P.trace_steps = ctx->trace_steps;
 
     const size_t np = np_of(ctx);
@@ -497,6 +503,27 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const bool prec = ctx->precise;
     int launches = 0;
 
+    if (ctx->scheme == 1) {
+        // The paper's ordering (Eq. 14-15): N(dz/2) - L(dz) - N(dz/2).  ROW_FIRST takes the first
+        // half-step of step 0, the row pass n of the loop the second half of step n and the first half of step
+        // n + 1, ROW_FINAL the second half of step nz - 1; every linear step is a full dz (tables 0).
+        if (!prec || P.Q) return SHG_EINVAL;     // this variant: hi+lo constants only, no heat output
+        CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 0, prec, grid_r, st)); ++launches;
+        CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
+        if (use_persist && g.nz > 1) {
+            const int grid_p = grid_r > grid_c ? grid_r : grid_c;
+            ctx->trace_grid = grid_p;
+            CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
+        } else {
+            for (int n = 0; n < g.nz - 1; ++n) {
+                CU(ctx->Lx.row(P, shg::ROW_MID, n, 0, prec, grid_r, st)); ++launches;
+                CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
+            }
+        }
+        if (ctx->timing) { CU(cudaEventRecord(ctx->ev[1], st)); ctx->ev_recorded = true; }
+        CU(ctx->Lx.row(P, shg::ROW_FINAL, g.nz - 1, 0, prec, grid_r, st)); ++launches;
+    } else {
     // opening half-step (x part) on the input, then its y part
     CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 1, prec, grid_r, st)); ++launches;
     CU(ctx->Ly.col(P, 1, prec, grid_c, st)); ++launches;
@@ -514,6 +541,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     }
     if (ctx->timing) { CU(cudaEventRecord(ctx->ev[1], st)); ctx->ev_recorded = true; }
     CU(ctx->Lx.row(P, shg::ROW_FINAL, 0, 0, prec, grid_r, st)); ++launches;
+    }
 
     ctx->last_stream = st;
     ctx->last_batch = batch;

@@ -488,6 +488,179 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 }
 
 // ------------------------------------------------------------------------------------------------
+// The paper's own ordering, Eq. 14-15:  N(dz/2) - L(dz) - N(dz/2)  per z-step (SHG_OPT_SCHEME = 1).
+// Two consecutive nonlinear half-steps meet in real space, so the row pass between the linear steps of z-step
+// n and n + 1 takes the second half of step n, records P_j(z_{n+1}) at the true node, and takes the first half
+// of step n + 1:
+//   ROW_FIRST : A_in -> P_j(0) -> N(dz/2) [step 0, first half] -> F_x -> * hx(dz)                     -> A
+//   ROW_MID   : A -> F_x -> conj -> N(dz/2) [step n, second] -> P_j(z_{n+1}) -> N(dz/2) [step n+1, first]
+//                 -> F_x -> * hx(dz)                                                                  -> A
+//   ROW_FINAL : A -> F_x -> conj -> N(dz/2) [step nz-1, second] -> P_j(L)                             -> A_out
+// The linear step is always a full dz (tables index 0); the column pass is the one of the merged scheme.
+// Phases inside a step (G15, dk linear in z):  phi(z_n + s) = phi_n + s dk_n + s^2 (dk_{n+1} - dk_n)/(2 dz),
+// sampled at s = 0, dz/4, dz/2 (first half) and dz/2, 3dz/4, dz (second half): RK4 of length dz/2 (G8).
+// A variant, not the benchmarked path: no software pipelining of the temperature loads.
+// ------------------------------------------------------------------------------------------------
+// Temperature rise at step node j for the point at idx (G15)
+__device__ __forceinline__ float dT_at_node(const float* __restrict__ Tb, size_t plane, size_t idx, const TNode& t,
+                                            float Thi, float Tlo) {
+    const float* p = Tb + (size_t)t.k * plane + idx;
+    const float t0 = __ldg(p);
+    const float t1 = t.two ? __ldg(p + plane) : 0.f;
+    return dT_lerp(t0, t1, t.f, t.two, Thi, Tlo);
+}
+
+// phase reduced to [-pi, pi] in double, returned as float (uniform temperature: phi = dk z exactly)
+__device__ __forceinline__ float wrapped_phase(double p) {
+    const double TWO_PI = 6.283185307179586476925286766559;
+    return (float)(p - TWO_PI * rint(p / TWO_PI));
+}
+
+template <int NX, int MODE, bool PREC>
+__device__ __forceinline__ void row_item_paper(const Params& P, int item, int n, float2* smem_cta,
+                                               const float4* __restrict__ tws, int warp, int lane) {
+    using GE = Geo<NX>;
+    constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
+    const int g = lane / M, m = lane % M;
+    const int f = (G >= 2) ? g / HG : (warp & 1);
+    const int r = (G >= 2) ? g % HG : 0;
+    const int row = item * HG + r;
+    const int b = (item * HG) / P.ny;
+    const int y = row - b * P.ny;
+    const size_t rbase = (size_t)row * NX;
+    float2* own = smem_cta + (size_t)warp * (G * NP) + g * NP;
+    float2* par = (G >= 2) ? smem_cta + (size_t)warp * (G * NP) + (g ^ HG) * NP
+                           : smem_cta + (size_t)(warp ^ 1) * (G * NP);
+    const MemberDev& mb = P.mem[b];
+    const int rot = f ? NX / 2 : 0;
+    float2 v[R];
+    float sin0 = 0.f;                                   // ROW_FIRST: sum |A|^2 of the input line
+
+    if constexpr (MODE == ROW_FIRST) {
+        const float2* src = f ? P.Ain[1] : P.Ain[0];
+        if (src) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = src[rbase + ((M * q + m + rot) & (NX - 1))];
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) sin0 += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
+    } else {
+        float2* A = (f ? P.A[1] : P.A[0]) + rbase;
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        warp_fft<NX, PREC>(v, own, tws, m);             // inverse along x of the previous linear step (conj trick)
+    }
+    // the line meets its partner field in shared memory (MID / FINAL: conj(field) is stored)
+#pragma unroll
+    for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
+    if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
+
+    // ---- nonlinear half-steps on elements e = M q + m + f N/2, q < R/2 (own lower half, partner's upper half)
+    float2* p1 = (f ? par + M * H : own) + m;
+    float2* p2 = (f ? own : par + M * H) + m;
+    constexpr bool DO_SECOND = (MODE != ROW_FIRST);     // second half of z-step n
+    constexpr bool DO_FIRST = (MODE != ROW_FINAL);      // first half of z-step n1
+    const int n1 = (MODE == ROW_FIRST) ? 0 : n + 1;
+    const float k1h = 0.5f * mb.kap1dz, k2h = 0.5f * mb.kap2dz, g1h = 0.5f * mb.g1dz, g2h = 0.5f * mb.g2dz;
+    float s1 = 0.f, s2 = 0.f;
+    if (P.nzt == 0) {
+        // uniform temperature: phi(z) = dk z exactly, all sampled phases are warp-uniform
+        PhaseCoef S[3], F[3];
+        const double z0 = (double)n * mb.dzd, z1 = (double)n1 * mb.dzd;
+        const double zs[3] = {z0 + 0.5 * mb.dzd, z0 + 0.75 * mb.dzd, z0 + mb.dzd};
+        const double zf[3] = {z1, z1 + 0.25 * mb.dzd, z1 + 0.5 * mb.dzd};
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            float c, sn;
+            if (DO_SECOND) { sincosf(wrapped_phase(mb.dk_uniform * zs[i]), &sn, &c); S[i] = phase_coef(c, sn, k1h, k2h); }
+            if (DO_FIRST) { sincosf(wrapped_phase(mb.dk_uniform * zf[i]), &sn, &c); F[i] = phase_coef(c, sn, k1h, k2h); }
+        }
+#pragma unroll 1
+        for (int q = 0; q < H; ++q) {
+            float2 a1 = p1[M * q], a2 = p2[M * q];
+            if (MODE != ROW_FIRST) { a1.y = -a1.y; a2.y = -a2.y; }
+            if (DO_SECOND) {
+                rk4_point(a1, a2, S[0], S[1], S[2], g1h, g2h);
+                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
+                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+            }
+            if (DO_FIRST) rk4_point(a1, a2, F[0], F[1], F[2], g1h, g2h);
+            p1[M * q] = a1;
+            p2[M * q] = a2;
+        }
+    } else {
+        const size_t plane = (size_t)P.ny * NX;
+        const size_t pbase = (size_t)y * NX + rot + m;
+        const float* Tb = P.T + (P.T_per_member ? (size_t)b * P.nzt * plane : 0);
+        float* phi = P.phi + (size_t)b * plane + pbase;
+        const TNode tn0 = t_node(n, P.nz, P.nzt), tn1 = t_node(n1, P.nz, P.nzt), tn2 = t_node(n1 + 1, P.nz, P.nzt);
+        const float dz = mb.dz, gT = mb.gT, dk0c = mb.dk0, Thi = mb.Tpm_hi, Tlo = mb.Tpm_lo;
+        auto half = [&](float2& a1, float2& a2, float pa, float pm, float pb) {
+            float ca, sa, cm, sm, cb, sb;
+            __sincosf(pa, &sa, &ca);
+            __sincosf(pm, &sm, &cm);
+            __sincosf(pb, &sb, &cb);
+            rk4_point(a1, a2, phase_coef(ca, sa, k1h, k2h), phase_coef(cm, sm, k1h, k2h),
+                      phase_coef(cb, sb, k1h, k2h), g1h, g2h);
+        };
+#pragma unroll 1
+        for (int q = 0; q < H; ++q) {
+            const size_t idx = pbase + (size_t)(M * q);
+            float2 a1 = p1[M * q], a2 = p2[M * q];
+            if (MODE != ROW_FIRST) { a1.y = -a1.y; a2.y = -a2.y; }
+            float ph = __ldcg(phi + M * q);                                  // phi at node n (MID, FINAL) / 0 (FIRST)
+            float dkA = fmaf(gT, dT_at_node(Tb, plane, idx, tn1, Thi, Tlo), dk0c);   // dk at node n1
+            if (DO_SECOND) {
+                const float dk0 = fmaf(gT, dT_at_node(Tb, plane, idx, tn0, Thi, Tlo), dk0c);   // node n; dkA = node n+1
+                const float pa = fmaf(0.125f * dz, fmaf(3.0f, dk0, dkA), ph);
+                const float pm = fmaf(0.03125f * dz, fmaf(15.0f, dk0, 9.0f * dkA), ph);
+                const float pb = fmaf(0.5f * dz, dk0 + dkA, ph);
+                half(a1, a2, pa, pm, pb);
+                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
+                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+                ph = wrap_2pi(pb);
+                __stcg(phi + M * q, ph);                                     // phi at node n + 1
+            }
+            if (DO_FIRST) {
+                const float dkB = fmaf(gT, dT_at_node(Tb, plane, idx, tn2, Thi, Tlo), dk0c);   // node n1 + 1
+                const float pm = fmaf(0.03125f * dz, fmaf(7.0f, dkA, dkB), ph);
+                const float pb = fmaf(0.125f * dz, fmaf(3.0f, dkA, dkB), ph);
+                half(a1, a2, ph, pm, pb);
+            }
+            p1[M * q] = a1;
+            p2[M * q] = a2;
+        }
+    }
+    // ---- powers at the true nodes (no Parseval factor: the fields are in real space at z_{n+1})
+    {
+        const float t1 = DO_SECOND ? s1 : (f ? 0.f : sin0), t2 = DO_SECOND ? s2 : (f ? sin0 : 0.f);
+        const float w1 = warp_sum(t1), w2 = warp_sum(t2);
+        if (lane == 0) {
+            double* hst = P.hist + ((size_t)b * (P.nz + 1) + (DO_SECOND ? n + 1 : 0)) * 2;
+            if (DO_SECOND || G >= 2 || f == 0) atomicAdd(hst + 0, (double)w1 * mb.pscale_in[0]);
+            if (DO_SECOND || G >= 2 || f == 1) atomicAdd(hst + 1, (double)w2 * mb.pscale_in[1]);
+        }
+    }
+    if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
+#pragma unroll
+    for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
+    if constexpr (MODE == ROW_FINAL) {
+        float2* A = (f ? P.A[1] : P.A[0]) + rbase;
+#pragma unroll
+        for (int q = 0; q < R; ++q) stcg2(A + ((M * q + m + rot) & (NX - 1)), v[q]);
+    } else {
+        __syncwarp();
+        warp_fft<NX, PREC>(v, own, tws, m);
+        table_mul<R, M, PREC, false>(v, P.hx[0] + ((size_t)b * 2 + f) * NX + m);
+        float2* dst = (f ? P.A[1] : P.A[0]) + rbase;
+#pragma unroll
+        for (int q = 0; q < R; ++q) stcg2(dst + M * q + m, v[q]);
+    }
+}
+// ------------------------------------------------------------------------------------------------
 // Forward transform of SC = 8 adjacent columns by a team of TW = M/4 warps ("tile" layout).  Thread
 // (c, t) -- lane = 8 j + c, t = 4 (warp rank in team) + j -- holds, for column c, the elements t + M q,
 // q = 0..R-1, in v[q]: the same strided layout in and out as warp_fft, but the M residues of a column sit
@@ -611,6 +784,18 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
         row_item<NX, MODE, PREC, HEAT>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
 
+template <int NX, int MODE, bool PREC>
+__device__ __forceinline__ void row_pass_paper(const Params& P, int n, float2* smem_cta,
+                                               const float4* __restrict__ tws, int warp, int lane) {
+    using GE = Geo<NX>;
+    int lo, hi;
+    cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
+    const int slot = (GE::G >= 2) ? warp : (warp >> 1);
+    if (slot >= P.row_slots) return;
+    for (int it = lo + slot; it < hi; it += P.row_slots)
+        row_item_paper<NX, MODE, PREC>(P, it, n, smem_cta, tws, warp, lane);
+}
+
 template <int NY, bool PREC, int NXC>
 __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane) {
@@ -633,6 +818,14 @@ __global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row(Params P, int n, in
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
     row_pass<NX, MODE, PREC, HEAT>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
+}
+
+template <int NX, int MODE, bool PREC>
+__global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row_paper(Params P, int n) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
+    row_pass_paper<NX, MODE, PREC>(P, n, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 template <int NY, bool PREC>
@@ -713,6 +906,24 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
         row_pass<N, ROW_MID, PREC, HEAT>(P, n, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
+        if (!grid_barrier(P, epoch, n, 1)) return;
+    }
+}
+
+// The paper's ordering (SHG_OPT_SCHEME = 1): the loop body is "second half of step n, first half of step n + 1",
+// then the linear step of step n + 1 along y; n = 0 .. nz - 2 (ROW_FIRST / ROW_FINAL take the outer half-steps).
+template <int N, bool PREC>
+__global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_paper(Params P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const float4* tws = load_twiddles<N>(smem_raw, P.twx);
+    float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
+    unsigned int epoch = 0;
+#pragma unroll 1
+    for (int n = 0; n < P.nz - 1; ++n) {
+        row_pass_paper<N, ROW_MID, PREC>(P, n, smem_cta, tws, warp, lane);
+        if (!grid_barrier(P, epoch, n, 0)) return;
+        col_pass<N, PREC, N>(P, 0, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;
     }
 }

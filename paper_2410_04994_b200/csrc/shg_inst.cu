@@ -26,6 +26,14 @@ cudaError_t launch_row_t(const Params& P, int n, int hsel, int grid, cudaStream_
     return cudaGetLastError();
 }
 
+template <int MODE>
+cudaError_t launch_row_paper_t(const Params& P, int n, int grid, cudaStream_t st) {
+    cudaError_t e = set_smem(k_row_paper<N, MODE, true>, GE::CTA_SMEM);
+    if (e != cudaSuccess) return e;
+    k_row_paper<N, MODE, true><<<grid, GE::THREADS, GE::CTA_SMEM, st>>>(P, n);
+    return cudaGetLastError();
+}
+
 template <bool PREC>
 cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
     cudaError_t e = set_smem(k_col<N, PREC>, GE::CTA_SMEM);
@@ -55,6 +63,11 @@ cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
 
 cudaError_t SHG_CAT(launch_row_, SHG_N)(const Params& P, int mode, int n, int hsel, bool prec, int grid,
                                         cudaStream_t st) {
+    if (P.scheme == 1) {          // the paper's ordering: hi+lo constants only, full-step tables
+        if (mode == ROW_FIRST) return launch_row_paper_t<ROW_FIRST>(P, n, grid, st);
+        if (mode == ROW_MID) return launch_row_paper_t<ROW_MID>(P, n, grid, st);
+        return launch_row_paper_t<ROW_FINAL>(P, n, grid, st);
+    }
     if (prec) {
         if (mode == ROW_FIRST) return launch_row_t<ROW_FIRST, true>(P, n, hsel, grid, st);
         if (mode == ROW_MID) return P.Q ? launch_row_t<ROW_MID, true, true>(P, n, hsel, grid, st)
@@ -73,6 +86,15 @@ cudaError_t SHG_CAT(launch_col_, SHG_N)(const Params& P, int hsel, bool prec, in
 }
 
 cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid, cudaStream_t st) {
+    if (P.scheme == 1) {
+        const int smem = GE::CTA_SMEM;
+        cudaError_t e = set_smem(k_persist_paper<N, true>, smem);
+        if (e != cudaSuccess) return e;
+        Params Pc = P;
+        void* args[] = {&Pc};
+        return cudaLaunchCooperativeKernel((const void*)k_persist_paper<N, true>, dim3(grid), dim3(GE::THREADS), args,
+                                           (size_t)smem, st);
+    }
     if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
 }

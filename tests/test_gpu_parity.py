@@ -441,3 +441,54 @@ def test_walk_off_matches_oracle():
     w0 = dict(w, crystal=dict(c, rho1=0.0, rho2=0.0))
     z1, z2, _, _ = run_gpu(w0)
     assert rel_l2(g2, z2) > 1e-2                                      # the angles matter at this size
+
+
+# ------------------------------------------------------------------------------------------------
+# the paper's own ordering N/2 - L - N/2 (Eq. 14-15): SHG_OPT_SCHEME = 1 vs the oracle's scheme 1
+# ------------------------------------------------------------------------------------------------
+def run_gpu_scheme1(w, persistent=True):
+    g = dict(w["grid"])
+    ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=persistent)
+    ctx.set_option(shg.OPT_SCHEME, 1)
+    if g["nzt"] > 0:
+        ctx.set_temperature(torch.from_numpy(w["T"]).cuda(), per_member=w["per_member"])
+    else:
+        ctx.set_temperature(None, w["T_uniform"])
+    A1 = torch.from_numpy(w["A1"]).cuda()
+    o1, o2 = ctx.propagate(A1)
+    torch.cuda.synchronize()
+    return o1.cpu().numpy(), o2.cpu().numpy(), [ctx.power_history(b) for b in range(A1.shape[0])], ctx
+
+
+def run_oracle_scheme1(w):
+    g = dict(w["grid"])
+    o = oracle.Oracle(g, w["crystal"], w["beams"], scheme=1)
+    o.set_temperature(w["T"], w["T_uniform"], w["per_member"])
+    a1, a2 = o.propagate(w["A1"].astype(np.complex128))
+    return a1, a2, [o.power_history(b) for b in range(g["batch"])]
+
+
+@pytest.mark.parametrize("name,nz,kw", [("cfg1", 40, {}), ("cfg2", 30, {}), ("cfg3", 9, {}), ("cfg5", 6, {}),
+                                        ("cfg4", 12, {"batch": 5}), ("cfg2", 1, {}), ("cfg2", 2, {})])
+def test_paper_ordering_matches_oracle_scheme1(name, nz, kw):
+    w = wl.make(name, nz=nz, **kw)
+    g1, g2, gh, ctx = run_gpu_scheme1(w)
+    o1, o2, oh = run_oracle_scheme1(w)
+    check(w, g1, g2, gh, o1, o2, oh, tol_field=2e-5, tol_eta=2e-5)
+    # the two orderings are different schemes: the GPU must follow the one it was asked for
+    z1, z2, zh = run_oracle(w)
+    if nz >= 9 and name != "cfg4":
+        assert rel_l2(o2, z2) > 10 * rel_l2(g2, o2)
+
+
+def test_paper_ordering_launch_schemes_agree_and_argument_errors():
+    w = wl.make("cfg2", nz=20)
+    a1, a2, ah, ca = run_gpu_scheme1(w, persistent=True)
+    b1, b2, bh, cb = run_gpu_scheme1(w, persistent=False)
+    assert ca.last_launch_count() == 4 and cb.last_launch_count() == 3 + 2 * (20 - 1)
+    assert np.array_equal(a1, b1) and np.array_equal(a2, b2)
+    ca.set_option(shg.OPT_PRECISE, 0)
+    with pytest.raises(shg.ShgError):
+        ca.propagate(torch.from_numpy(w["A1"]).cuda())
+    with pytest.raises(shg.ShgError):
+        ca.set_option(shg.OPT_SCHEME, 2)
