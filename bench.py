@@ -169,6 +169,19 @@ def time_oracle_sample(w_full, budget_s: float, nz_probe: int = 1):
     return npts * nz_s / dt, oracle.num_threads(), desc, dt
 
 
+def cpu_context():
+    """Host CPU model and the oracle's build line, for the reported CPU baseline."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count(), "build": "gcc -O2 -std=c99 -fopenmp (no -ffast-math)"}
+
+
 def _with_nz(w, nz_s):
     """Same workload with a different z-step count.  Configs whose T planes sit on the step nodes (nzt = nz+1)
     are regenerated; a fixed-plane-count T (cfg5) is reused as is (it is interpolated in z)."""
@@ -205,7 +218,8 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_label(w), "nx": g["nx"], "ny": g["ny"], "nz": g["nz"], "batch": g["batch"],
                    "nzt": g["nzt"]},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": dict({"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+                             **cpu_context()),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -368,6 +382,14 @@ def run_b200(args):
         oracle.build()
         v, cores, desc, dt = time_oracle_sample(w, 15.0)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        cpu.update(cpu_context())
+        # the same oracle on one thread (single-thread and all-core figures), a shorter sample
+        oracle.set_num_threads(1)
+        try:
+            v1, _, desc1, _ = time_oracle_sample(w, 6.0)
+        finally:
+            oracle.set_num_threads(cores)
+        cpu["single_thread"] = {"value": v1, "sample": desc1}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -11,4 +11,5 @@ from .oracle import (  # noqa: F401
     fft2,
     gaussian_input,
     num_threads,
+    set_num_threads,
 )

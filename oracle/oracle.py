@@ -67,11 +67,17 @@ def _load():
     lib.orc_destroy.argtypes = [C.c_void_p]
     lib.orc_destroy.restype = None
     lib.orc_gaussian_input.argtypes = [C.POINTER(Grid), C.POINTER(Crystal), C.POINTER(Beam), C.c_void_p]
+    lib.orc_set_num_threads.argtypes = [C.c_int]
+    lib.orc_set_num_threads.restype = None
     lib.orc_fft2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
     lib.orc_dft2_brute.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]
     lib.orc_num_threads.restype = C.c_int
     _lib = lib
     return lib
+
+
+def set_num_threads(n: int) -> None:
+    _load().orc_set_num_threads(int(n))
 
 
 def num_threads() -> int:

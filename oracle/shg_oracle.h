@@ -95,6 +95,7 @@ int  orc_fft2(double* data, int ny, int nx, int sign);
 int  orc_dft2_brute(const double* in, double* out, int ny, int nx, int sign);
 
 int  orc_num_threads(void);
+void orc_set_num_threads(int n);   /* OpenMP threads of the following calls (timing the oracle on one core) */
 
 #ifdef __cplusplus
 }
