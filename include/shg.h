@@ -74,8 +74,11 @@ typedef struct {
 
 /* Options for shg_set_option. */
 #define SHG_OPT_PERSISTENT 1   /* 1 (default): one persistent cooperative kernel runs the whole z-loop with
-                                  device-wide barriers between the row and column passes (square grids);
-                                  0: two ordinary kernel launches per z-step (any nx, ny).              */
+                                  device-wide barriers between the row and column passes (square grids; if
+                                  the device cannot make all its CTAs co-resident -- SMs held by another
+                                  context, MPS / MIG -- the call falls back to the scheme of value 0);
+                                  0: two ordinary kernel launches per z-step (any nx, ny).  Same device code,
+                                  bit-identical fields.                                                  */
 #define SHG_OPT_PRECISE    2   /* 1 (default): every reused constant (FFT twiddles, propagator tables) is an
                                   fp32 hi+lo pair whose lo part enters the FMA addend, so constant rounding
                                   does not accumulate linearly over thousands of z-steps; 0: plain fp32.  */

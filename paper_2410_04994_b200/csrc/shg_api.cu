@@ -280,6 +280,17 @@ void free_ctx(shg_ctx* ctx) {
     delete ctx;
 }
 
+// The persistent kernel needs every CTA co-resident (cooperative launch).  When the device cannot grant that
+// (SMs taken by another context, MPS / MIG slices, cooperative launch unsupported) the z-loop falls back to
+// two ordinary launches per z-step -- the same device code, bit-identical fields.
+bool coop_unavailable(cudaError_t e) {
+    if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources || e == cudaErrorNotSupported) {
+        cudaGetLastError();      // clear the sticky-free launch error
+        return true;
+    }
+    return false;
+}
+
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace
@@ -511,11 +522,15 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 0, prec, grid_r, st)); ++launches;
         CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
         if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
+        bool looped = false;
         if (use_persist && g.nz > 1) {
             const int grid_p = grid_r > grid_c ? grid_r : grid_c;
             ctx->trace_grid = grid_p;
-            CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
-        } else {
+            const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
+            if (e == cudaSuccess) { ++launches; looped = true; }
+            else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
+        }
+        if (!looped) {
             for (int n = 0; n < g.nz - 1; ++n) {
                 CU(ctx->Lx.row(P, shg::ROW_MID, n, 0, prec, grid_r, st)); ++launches;
                 CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
@@ -528,11 +543,15 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 1, prec, grid_r, st)); ++launches;
     CU(ctx->Ly.col(P, 1, prec, grid_c, st)); ++launches;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
+    bool looped = false;
     if (use_persist) {
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
         ctx->trace_grid = grid_p;
-        CU(ctx->Lx.persist(P, prec, grid_p, st)); ++launches;
-    } else {
+        const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
+        if (e == cudaSuccess) { ++launches; looped = true; }
+        else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
+    }
+    if (!looped) {
         for (int n = 0; n < g.nz; ++n) {
             const int hsel = (n == g.nz - 1) ? 1 : 0;
             CU(ctx->Lx.row(P, shg::ROW_MID, n, hsel, prec, grid_r, st)); ++launches;
