@@ -5,8 +5,8 @@
 // One line of length N = R * M is held by M lanes (R values per lane, G = 32/M lines per warp).
 // Decomposition  n = M n1 + n2 (lane n2 = m holds n1 = 0..R-1),  k = k1 + R k2:
 //   X[k1 + R k2] = sum_{n2} W_M^{n2 k2} [ W_N^{n2 k1} sum_{n1} W_R^{n1 k1} x[M n1 + n2] ]
-// stage A: radix-R in registers; twiddle W_N^{k1 m}; one transpose through shared memory (XOR-swizzled,
-// conflict free); stage B: R/M radix-M FFTs in registers.  Input and output are both "strided": lane m holds
+// stage A: radix-R in registers; twiddle W_N^{k1 m}; one transpose through shared memory (padded line,
+// pitch M + 1: conflict free); stage B: R/M radix-M FFTs in registers.  Input and output are both "strided": lane m holds
 // elements m + M q, q = 0..R-1 -- which is also the coalesced global layout.
 //
 // Only the FORWARD transform exists in the code (one instance keeps the z-loop inside the instruction
