@@ -18,9 +18,13 @@
  *   TPA                 vs I0/(1+beta I0 z)
  *   temperature/phase   vs sinc^2 with dk = dk0 + g dT for every nzt encoding of the same field,
  *                       and the closed form for a linear-in-z mismatch
- * The complete path with everything switched on at once (diffraction + coupling + T + TPA, the five
- * BASELINE configs) has no closed form and no paper-printed value: for those runs "parity unpinned"
- * beyond the component pins above and dz-refinement self-convergence.
+ *   walk-off            vs an exact translation by whole cells and the centroid law tan(rho) z
+ *   heat source         vs alpha I0 e^{-alpha z}, beta I^2 of the TPA closed form, and P(0) - P(L) = integral of q
+ *   the complete path   (diffraction + walk-off + coupling + depletion + temperature-dependent mismatch +
+ *                       absorption + TPA at once) vs an independent solver of Eq. 2 written in the test (method
+ *                       of lines in the interaction picture, numpy FFT, scipy DOP853 at 1e-11): second-order
+ *                       convergence in dz, Richardson-extrapolated fields within 5e-8 (measured 3e-9, 6e-9).
+ * No value printed in the paper exists for the five BASELINE configs themselves (the paper prints none).
  */
 #ifndef SHG_ORACLE_H
 #define SHG_ORACLE_H

@@ -522,3 +522,90 @@ def test_walk_off_translates_the_beam_along_x_only():
     x, _y = wl.axes(n, n, bm)
     cen = lambda a: float((np.abs(a) ** 2 * x[None, :]).sum() / (np.abs(a) ** 2).sum())
     assert abs((cen(q1[0]) - cen(r1[0])) / (math.tan(1.3e-3) * c["L"]) - 1) < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------
+# 15. the COMPLETE path at once (diffraction + walk-off + coupling + depletion + temperature-dependent mismatch +
+#     absorption + two-photon absorption) against an independent solver of Eq. 2: method of lines in the
+#     interaction picture, numpy FFT, adaptive 8th-order Runge-Kutta (scipy DOP853) at tight tolerance.  Nothing
+#     below comes from the oracle: the equations are retyped from the paper with the readings of DESIGN.md §3.
+#     The split-step scheme must converge to it at second order in dz.
+# ------------------------------------------------------------------------------------------------
+def reference_solution(c, bm, n, A1_in, A2_in, Tplanes):
+    """A1(L), A2(L) of  dA1/dz = L1 A1 + i kappa1 A2 conj(A1) e^{-i phi} - (beta1/2) I1 A1,
+                        dA2/dz = L2 A2 + i kappa2 A1^2 e^{+i phi}        - (beta2/2) I2 A2,
+    L_j = -i k_perp^2/(2 k_j) - i kx tan(rho_j) - alpha_j/2 in Fourier space,  I_j = eps0 c n_j |A_j|^2 / 2,
+    phi(x,y,z) = int_0^z [dk0 + ddk_dT (T(x,y,z') - T_pm)] dz' with T linear in z between its planes."""
+    L = c["L"]
+    k1 = 2 * np.pi * c["n1"] / c["lambda1"]
+    k2 = 2 * np.pi * c["n2"] / (c["lambda1"] / 2)
+    kap1 = 2 * np.pi * c["d_eff"] / (c["n1"] * c["lambda1"])
+    kap2 = 2 * np.pi * c["d_eff"] / (c["n2"] * c["lambda1"])
+    c1, c2 = EPS0 * C0 * c["n1"] / 2, EPS0 * C0 * c["n2"] / 2
+    kx = 2 * np.pi * np.fft.fftfreq(n, d=bm["lx"] / n)[None, :]
+    ky = 2 * np.pi * np.fft.fftfreq(n, d=bm["ly"] / n)[:, None]
+    kp2 = kx ** 2 + ky ** 2
+    lin1 = -1j * kp2 / (2 * k1) - 1j * kx * math.tan(c["rho1"]) - c["alpha1"] / 2
+    lin2 = -1j * kp2 / (2 * k2) - 1j * kx * math.tan(c["rho2"]) - c["alpha2"] / 2
+    nzt = Tplanes.shape[0]
+    zk = np.linspace(0.0, L, nzt)
+    dk_k = c["dk0"] + c["ddk_dT"] * (Tplanes.astype(np.float64) - c["T_pm"])         # [nzt][n][n]
+    hk = L / (nzt - 1)
+    phi_k = np.concatenate([np.zeros((1, n, n)), np.cumsum(0.5 * (dk_k[1:] + dk_k[:-1]) * hk, axis=0)])
+
+    def phi(z):
+        k = min(int(z / hk), nzt - 2)
+        s = z - zk[k]
+        return phi_k[k] + dk_k[k] * s + (dk_k[k + 1] - dk_k[k]) * s * s / (2 * hk)
+
+    def rhs(z, y):
+        b1 = y[:n * n].reshape(n, n)
+        b2 = y[n * n:].reshape(n, n)
+        a1 = np.fft.ifft2(np.exp(lin1 * z) * b1)
+        a2 = np.fft.ifft2(np.exp(lin2 * z) * b2)
+        e = np.exp(1j * phi(z))
+        n1 = 1j * kap1 * a2 * np.conj(a1) / e - 0.5 * c["beta1"] * c1 * np.abs(a1) ** 2 * a1
+        n2 = 1j * kap2 * a1 * a1 * e - 0.5 * c["beta2"] * c2 * np.abs(a2) ** 2 * a2
+        return np.concatenate([(np.exp(-lin1 * z) * np.fft.fft2(n1)).ravel(), (np.exp(-lin2 * z) * np.fft.fft2(n2)).ravel()])
+
+    y0 = np.concatenate([np.fft.fft2(A1_in).ravel(), np.fft.fft2(A2_in).ravel()])
+    scale = np.abs(y0).max()
+    sol = integrate.solve_ivp(rhs, (0.0, L), y0, method="DOP853", rtol=1e-11, atol=1e-13 * scale)
+    assert sol.success
+    y = sol.y[:, -1]
+    return (np.fft.ifft2(np.exp(lin1 * L) * y[:n * n].reshape(n, n)),
+            np.fft.ifft2(np.exp(lin2 * L) * y[n * n:].reshape(n, n)))
+
+
+def test_complete_path_converges_to_an_independent_solver_of_eq2():
+    n, nzt = 32, 6
+    c = wl.crystal(8e-3, alpha=True, alpha1=3.0, alpha2=20.0, beta1=1e-11, beta2=6e-11, dk0=35.0, ddk_dT=-150.0,
+                   rho1=-0.4e-3, rho2=0.9e-3)
+    bm = wl.beam(c, 250.0, 1.1, 9.0, focus_z=0.6 * c["L"])
+    bm["ly"] = 1.15 * bm["lx"]
+    rng = np.random.default_rng(15)
+    x, y = wl.axes(n, n, bm)
+    A1 = np.roll(wl.gaussian_pump(n, n, c, bm), (2, -1), axis=(0, 1)).astype(np.complex128)
+    A2 = 0.05 * np.roll(A1, 3, axis=1) * np.exp(0.4j)
+    # smooth asymmetric temperature planes (the mismatch phase varies by several rad across the beam and along z)
+    T = np.empty((nzt, n, n), dtype=np.float32)
+    for k in range(nzt):
+        T[k] = (wl.T_PM + 1.5 * np.exp(-((x[None, :] - 0.2 * bm["w0"]) ** 2 + (y[:, None] + 0.1 * bm["w0"]) ** 2)
+                                       / (1.5 * bm["w0"]) ** 2) * (0.3 + 0.2 * k) + 0.05 * rng.standard_normal())
+    r1, r2 = reference_solution(c, bm, n, A1, A2, T)
+    assert np.linalg.norm(r2) / np.linalg.norm(r1) > 0.15          # a strongly converting, depleting case
+    errs = []
+    sols = []
+    for nz in (40, 80, 160):                                        # plane knots sit on step nodes (5 divides nz)
+        o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=nzt), c, [bm])
+        o.set_temperature(T, 0.0, False)
+        o1, o2 = o.propagate(A1[None], A2[None])
+        sols.append((o1[0], o2[0]))
+        errs.append((rel_l2(o1[0], r1), rel_l2(o2[0], r2)))
+    for j in (0, 1):
+        assert 3.5 < errs[0][j] / errs[1][j] < 4.5 and 3.5 < errs[1][j] / errs[2][j] < 4.5, errs   # second order
+        assert errs[2][j] < 3e-5, errs
+    # Richardson extrapolation of the two finest runs removes the dz^2 term: what is left is the oracle's own error
+    e1 = (4 * sols[2][0] - sols[1][0]) / 3
+    e2 = (4 * sols[2][1] - sols[1][1]) / 3
+    assert rel_l2(e1, r1) < 5e-8 and rel_l2(e2, r2) < 5e-8, (rel_l2(e1, r1), rel_l2(e2, r2))   # measured 3e-9, 6e-9
