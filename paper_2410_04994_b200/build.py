@@ -3,7 +3,8 @@
     python -m paper_2410_04994_b200.build [--force] [--verbose]
 
 One object per line length (64..1024) plus the host API, compiled in parallel, linked into
-``paper_2410_04994_b200/libshg.so``.  nvcc cross-compiles without a GPU.
+``paper_2410_04994_b200/libshg.so``.  nvcc cross-compiles without a GPU.  Environment: ``NVCC`` (compiler
+path), ``SHG_NVCC_EXTRA`` (extra nvcc flags, e.g. ``-Xptxas -v`` or a ``-D`` for an experiment).
 """
 from __future__ import annotations
 
