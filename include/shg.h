@@ -8,6 +8,7 @@
  * What one call to shg_propagate computes, per batch member (members are independent):
  *   for n = 0 .. nz-1:                                  dz = L/nz
  *     A_j <- F^-1{ exp(-i(kx^2+ky^2)(dz/2)/(2k_j) - alpha_j dz/4) F{A_j} }, j = 1,2    (G3)
+ *            (with walk-off angles: one more factor exp(-i kx tan(rho_j) dz/2), G21)
  *     one classical RK4 step of length dz, independently at every (x,y), of              (Eq. 2, G2, G5)
  *        dA1/dz = i kappa1 A2 conj(A1) e^{-i phi} - (beta1/2) I1 A1
  *        dA2/dz = i kappa2 A1^2        e^{+i phi} - (beta2/2) I2 A2,   I_j = eps0 c n_j |A_j|^2 / 2
