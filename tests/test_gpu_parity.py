@@ -492,3 +492,73 @@ def test_paper_ordering_launch_schemes_agree_and_argument_errors():
         ca.propagate(torch.from_numpy(w["A1"]).cuda())
     with pytest.raises(shg.ShgError):
         ca.set_option(shg.OPT_SCHEME, 2)
+
+
+# ------------------------------------------------------------------------------------------------
+# guard bands: every caller-owned array sits inside a larger allocation whose surroundings hold NaN (inputs) or a
+# sentinel (outputs); a read outside would poison the result, a write outside would damage the sentinel
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,nz,kw", [("cfg2", 5, {}), ("cfg2", 5, {"scheme": 1}), ("cfg2", 6, {"heat": 4}),
+                                        ("cfg3", 3, {}), ("cfg5", 3, {}), ("cfg4", 4, {"batch": 3}),
+                                        ("cfg2", 4, {"persistent": False, "scheme": 1}), ("cfg1", 4, {"heat": 1})])
+def test_no_access_outside_the_callers_arrays(name, nz, kw):
+    kw = dict(kw)
+    scheme, heat, persistent = kw.pop("scheme", 0), kw.pop("heat", 0), kw.pop("persistent", True)
+    w = wl.make(name, nz=nz, **kw)
+    g = dict(w["grid"])
+    PAD = 4096                                                     # elements on either side (16-byte aligned)
+
+    def guarded(arr, fill):
+        flat = torch.from_numpy(np.ascontiguousarray(arr)).reshape(-1)
+        big = torch.full((flat.numel() + 2 * PAD,), fill, dtype=flat.dtype, device="cuda")
+        big[PAD:PAD + flat.numel()] = flat.cuda()
+        return big, big[PAD:PAD + flat.numel()].view(*arr.shape)
+
+    def run(guard):
+        ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=persistent)
+        ctx.set_option(shg.OPT_SCHEME, scheme)
+        keep = []
+        nanc = complex(float("nan"), float("nan"))
+        if g["nzt"] > 0:
+            if guard:
+                bigT, Tv = guarded(w["T"], float("nan")); keep.append(bigT)
+            else:
+                Tv = torch.from_numpy(w["T"]).cuda()
+            ctx.set_temperature(Tv, per_member=w["per_member"])
+        else:
+            ctx.set_temperature(None, w["T_uniform"])
+        if guard:
+            bigA, Av = guarded(w["A1"], nanc); keep.append(bigA)
+        else:
+            Av = torch.from_numpy(w["A1"]).cuda()
+        outs = []
+        for _ in range(2):
+            if guard:
+                big, v = guarded(np.zeros_like(w["A1"]), complex(7.0, -7.0)); keep.append(big)
+            else:
+                v = torch.zeros_like(Av)
+            outs.append(v)
+        Q = None
+        if heat:
+            qshape = (g["batch"], heat, g["ny"], g["nx"])
+            if guard:
+                bigQ, Q = guarded(np.zeros(qshape, dtype=np.float32), 7.0); keep.append(bigQ)
+            else:
+                Q = torch.zeros(qshape, dtype=torch.float32, device="cuda")
+            ctx.set_heat_output(Q)
+        ctx.propagate(Av, None, outs[0], outs[1])
+        torch.cuda.synchronize()
+        hist = ctx.power_history(0)
+        return outs[0].cpu().numpy(), outs[1].cpu().numpy(), hist, (None if Q is None else Q.cpu().numpy()), keep
+
+    r1, r2, rh, rq, _ = run(False)
+    g1, g2, gh, gq, keep = run(True)
+    assert np.isfinite(g1).all() and np.isfinite(g2).all()
+    assert np.array_equal(g1, r1) and np.array_equal(g2, r2)       # no NaN from outside got in
+    if heat:
+        assert np.array_equal(gq, rq)
+    for big in keep:                                               # guard zones untouched
+        head, tail = big[:PAD].cpu().numpy(), big[-PAD:].cpu().numpy()
+        for z in (head, tail):
+            assert np.all((z == z[0]) | (z != z)), "guard zone modified"
+            assert (z != z).all() or z[0] in (7.0, complex(7.0, -7.0))
