@@ -513,6 +513,14 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     }
     const bool prec = ctx->precise;
     int launches = 0;
+    {   // Sparse launch: every CTA owns at most one row item per slot and at most half of its warps have one
+        // (single small simulations).  The persistent kernel then spreads the nonlinear step over the whole CTA.
+        const int grid_p = grid_r > grid_c ? grid_r : grid_c;
+        const int ipc = (UR + grid_p - 1) / grid_p;
+        const int warps_per_slot = ix.warps / ix.row_slots;
+        P.flat_rows = (use_persist && ctx->scheme == 0 && !P.Q && ipc <= ix.row_slots &&
+                       2 * ipc * warps_per_slot <= ix.warps) ? 1 : 0;
+    }
 
     if (ctx->scheme == 1) {
         // The paper's ordering (Eq. 14-15): N(dz/2) - L(dz) - N(dz/2).  ROW_FIRST takes the first

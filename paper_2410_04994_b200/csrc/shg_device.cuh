@@ -784,6 +784,128 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
         row_item<NX, MODE, PREC, HEAT>(P, it, n, hsel, smem_cta, tws, warp, lane);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Row pass of a z-step for SPARSE launches: a CTA owns at most one item per slot and at most half of its warps
+// have one (single small simulations: cfg1-cfg3 give an SM one or two rows).  The transforms stay with the
+// warps that own the rows, but the nonlinear step of the CTA's rows is dealt point by point to all 512 threads
+// (one or two points per thread instead of R/2 per lane of one warp): the RK4 chain, half of a row item's
+// latency, leaves the critical path.  Same per-point arithmetic as row_item<ROW_MID>: bit-identical fields.
+//   phase A  owners: load -> F_x -> line to shared memory          | __syncthreads
+//   phase B  everyone: T / phase / RK4 on the CTA's points, power sums into shared accumulators | __syncthreads
+//   phase C  one thread per (row, field): power to the history;  owners: F_x -> * hx -> store
+// ------------------------------------------------------------------------------------------------
+template <int NX, bool PREC>
+__device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, float2* smem_cta,
+                                              const float4* __restrict__ tws, int warp, int lane, double* s_acc) {
+    using GE = Geo<NX>;
+    constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG;
+    int lo, hi;
+    cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
+    const int nitems = hi - lo;                               // <= ROW_SLOTS (the host selects this pass only then)
+    const int slot = (G >= 2) ? warp : (warp >> 1);
+    const bool has = slot < nitems;
+    const int g = lane / M, m = lane % M;
+    const int f = (G >= 2) ? g / HG : (warp & 1);
+    const int r = (G >= 2) ? g % HG : 0;
+    float2* own = smem_cta + (size_t)warp * (G * NP) + g * NP;
+    float2 v[R];
+    float2* A = nullptr;
+    const float4* hx = nullptr;
+    if (has) {
+        const int item = lo + slot;
+        const int b = (item * HG) / P.ny;
+        A = (f ? P.A[1] : P.A[0]) + (size_t)(item * HG + r) * NX;
+        hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        table_prefetch<R, M>(hx, m);
+        warp_fft<NX, PREC>(v, own, tws, m);
+#pragma unroll
+        for (int q = 0; q < R; ++q) own[M * q + m] = v[q];     // conj(field), SH rotated by N/2
+    }
+    if (threadIdx.x < 2 * GE::ROW_SLOTS * HG) s_acc[threadIdx.x] = 0.0;
+    __syncthreads();
+
+    // ---- phase B: point idx = ((local item) * HG + row in item) * NX + e; a warp's 32 points share a row
+    const int total = nitems * HG * NX;
+    const size_t plane = (size_t)P.ny * NX;
+    const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
+    for (int idx = threadIdx.x; idx < total; idx += GE::THREADS) {
+        const int li = idx / (HG * NX), rr = (idx / NX) % HG, e = idx % NX;
+        float2* l1;
+        float2* l2;
+        if constexpr (G >= 2) {
+            l1 = smem_cta + (size_t)li * (G * NP) + rr * NP;             // group (f = 0, rr)
+            l2 = smem_cta + (size_t)li * (G * NP) + (HG + rr) * NP;      // group (f = 1, rr)
+        } else {
+            l1 = smem_cta + (size_t)(2 * li) * NP;
+            l2 = smem_cta + (size_t)(2 * li + 1) * NP;
+        }
+        float2* q1 = l1 + e;
+        float2* q2 = l2 + ((e + NX / 2) & (NX - 1));
+        const int row = (lo + li) * HG + rr;
+        const int b = row / P.ny, y = row - b * P.ny;
+        const MemberDev& mb = P.mem[b];
+        const float k1dz = mb.kap1dz, k2dz = mb.kap2dz;
+        float ca, sa, cm, sm, cb, sb;
+        if (P.nzt == 0) {
+            const double TWO_PI = 6.283185307179586476925286766559;
+            double pa = mb.dk_uniform * ((double)n * mb.dzd);
+            double pm = mb.dk_uniform * (((double)n + 0.5) * mb.dzd);
+            double pb = mb.dk_uniform * (((double)n + 1.0) * mb.dzd);
+            pa -= TWO_PI * rint(pa / TWO_PI);
+            pm -= TWO_PI * rint(pm / TWO_PI);
+            pb -= TWO_PI * rint(pb / TWO_PI);
+            sincosf((float)pa, &sa, &ca);
+            sincosf((float)pm, &sm, &cm);
+            sincosf((float)pb, &sb, &cb);
+        } else {
+            const float* Tb = P.T + (P.T_per_member ? (size_t)b * P.nzt * plane : 0);
+            const size_t pidx = (size_t)y * NX + e;
+            float* phi = P.phi + (size_t)b * plane + pidx;
+            const TPoint tp = t_load(Tb + (size_t)ta.k * plane, Tb + (size_t)tb.k * plane, plane, pidx, ta.two, tb.two, phi);
+            const float dTa = dT_lerp(tp.a0, tp.a1, ta.f, ta.two, mb.Tpm_hi, mb.Tpm_lo);
+            const float dTb = dT_lerp(tp.b0, tp.b1, tb.f, tb.two, mb.Tpm_hi, mb.Tpm_lo);
+            const float dka = fmaf(mb.gT, dTa, mb.dk0), dkb = fmaf(mb.gT, dTb, mb.dk0);
+            const float phm = fmaf(0.125f * mb.dz, fmaf(3.0f, dka, dkb), tp.ph);
+            const float phb = fmaf(0.5f * mb.dz, dka + dkb, tp.ph);
+            __sincosf(tp.ph, &sa, &ca);
+            __sincosf(phm, &sm, &cm);
+            __sincosf(phb, &sb, &cb);
+            __stcg(phi, wrap_2pi(phb));
+        }
+        const PhaseCoef CA = phase_coef(ca, sa, k1dz, k2dz), CM = phase_coef(cm, sm, k1dz, k2dz),
+                        CB = phase_coef(cb, sb, k1dz, k2dz);
+        float2 a1 = *q1, a2 = *q2;
+        a1.y = -a1.y; a2.y = -a2.y;
+        rk4_point(a1, a2, CA, CM, CB, mb.g1dz, mb.g2dz);
+        *q1 = a1;
+        *q2 = a2;
+        const float w1 = warp_sum(fmaf(a1.x, a1.x, a1.y * a1.y)), w2 = warp_sum(fmaf(a2.x, a2.x, a2.y * a2.y));
+        if (lane == 0) {
+            atomicAdd(&s_acc[(li * HG + rr) * 2 + 0], (double)w1);
+            atomicAdd(&s_acc[(li * HG + rr) * 2 + 1], (double)w2);
+        }
+    }
+    __syncthreads();
+
+    // ---- phase C
+    if ((int)threadIdx.x < nitems * HG * 2) {
+        const int row = lo * HG + (int)threadIdx.x / 2, fld = threadIdx.x & 1;
+        const int b = row / P.ny;
+        atomicAdd(P.hist + ((size_t)b * (P.nz + 1) + (n + 1)) * 2 + fld, s_acc[threadIdx.x] * P.mem[b].pscale_step[fld]);
+    }
+    if (has) {
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
+        __syncwarp();
+        warp_fft<NX, PREC>(v, own, tws, m);
+        table_mul<R, M, PREC, false>(v, hx + m);
+#pragma unroll
+        for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
+    }
+}
+
 template <int NX, int MODE, bool PREC>
 __device__ __forceinline__ void row_pass_paper(const Params& P, int n, float2* smem_cta,
                                                const float4* __restrict__ tws, int warp, int lane) {
@@ -904,6 +1026,25 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         row_pass<N, ROW_MID, PREC, HEAT>(P, n, hsel, smem_cta, tws, warp, lane);
+        if (!grid_barrier(P, epoch, n, 0)) return;
+        col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
+        if (!grid_barrier(P, epoch, n, 1)) return;
+    }
+}
+
+// Persistent kernel for sparse launches (see row_pass_flat).
+template <int N, bool PREC>
+__global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double s_acc[2 * Geo<N>::ROW_SLOTS * Geo<N>::HG];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const float4* tws = load_twiddles<N>(smem_raw, P.twx);
+    float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
+    unsigned int epoch = 0;
+#pragma unroll 1
+    for (int n = 0; n < P.nz; ++n) {
+        const int hsel = (n == P.nz - 1) ? 1 : 0;
+        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane, s_acc);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;

@@ -95,6 +95,15 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
         return cudaLaunchCooperativeKernel((const void*)k_persist_paper<N, true>, dim3(grid), dim3(GE::THREADS), args,
                                            (size_t)smem, st);
     }
+    if (P.flat_rows) {
+        const int smem = GE::CTA_SMEM;
+        const void* kf = prec ? (const void*)k_persist_flat<N, true> : (const void*)k_persist_flat<N, false>;
+        cudaError_t e = cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        Params Pc = P;
+        void* args[] = {&Pc};
+        return cudaLaunchCooperativeKernel(kf, dim3(grid), dim3(GE::THREADS), args, (size_t)smem, st);
+    }
     if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
 }

@@ -23,6 +23,7 @@ struct MemberDev {
 
 struct Params {
     int nx, ny, nz, nzt, batch;
+    int flat_rows;             // 1: sparse launch, the persistent kernel spreads the nonlinear step over the CTA (row_pass_flat)
     int scheme;                // 0: L/2 - N - L/2 with merged half-steps; 1: the paper's N/2 - L - N/2 (SHG_OPT_SCHEME)
     int acquire_fence;         // 1: gpu-scope acquire fence after every device-wide barrier (SHG_OPT_ACQUIRE_FENCE)
     int row_slots, col_teams;  // slots (warps / warp pairs) and teams per CTA that take items (<= Geo limits)

@@ -166,7 +166,9 @@ def test_persistent_and_per_pass_launches_agree(name, nz):
     b1, b2, bh, cb = run_gpu(w, persistent=False)
     assert ca.last_launch_count() == 4 and cb.last_launch_count() == 3 + 2 * nz
     assert np.array_equal(a1, b1) and np.array_equal(a2, b2)      # identical arithmetic, bit for bit
-    assert np.max(np.abs(ah[0] - bh[0])) <= 1e-12 * ah[0][0, 0]   # fp64 atomics: summation order only
+    # powers: fp32 partial sums per warp (grouped differently when the persistent kernel spreads the nonlinear
+    # step over the CTA, row_pass_flat), fp64 atomics in any order
+    assert np.max(np.abs(ah[0] - bh[0])) <= 1e-6 * ah[0][0, 0]
 
 
 @pytest.mark.parametrize("n", [64, 128, 256, 512, 1024])
