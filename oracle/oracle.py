@@ -35,7 +35,8 @@ class Beam(C.Structure):
 
 
 class Options(C.Structure):
-    _fields_ = [("scheme", C.c_int32), ("undepleted", C.c_int32), ("brute_dft", C.c_int32)]
+    _fields_ = [("scheme", C.c_int32), ("undepleted", C.c_int32), ("brute_dft", C.c_int32),
+                ("merged", C.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -128,7 +129,7 @@ class Oracle:
     """One oracle context: ``Oracle(grid, crystal, beams).set_temperature(...).propagate(A1, A2)``."""
 
     def __init__(self, grid: dict, crystal: dict, beams, scheme: int = 0, undepleted: bool = False,
-                 brute_dft: bool = False):
+                 brute_dft: bool = False, merged: bool = False):
         lib = _load()
         beams = list(beams)
         self.grid = dict(grid)
@@ -138,7 +139,7 @@ class Oracle:
         self.beams = beams
         g = _mk(Grid, self.grid)
         arr = (Beam * len(beams))(*[_mk(Beam, b) for b in beams])
-        opt = Options(int(scheme), int(bool(undepleted)), int(bool(brute_dft)))
+        opt = Options(int(scheme), int(bool(undepleted)), int(bool(brute_dft)), int(bool(merged)))
         h = C.c_void_p()
         rc = lib.orc_create(C.byref(g), C.byref(_mk(Crystal, crystal)), arr, C.byref(opt), C.byref(h))
         if rc:

@@ -370,6 +370,14 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
     const double hlin = (ctx->o.scheme == 0) ? 0.5 * dz : dz;
     cplx* H1 = linear_factor(g, bm, k1, c->alpha1, c->rho1, hlin);
     cplx* H2 = linear_factor(g, bm, k2, c->alpha2, c->rho2, hlin);
+    /* test aid (orc_options.merged, scheme 0 only): the closing half-step of z-step n and the opening half-step
+     * of z-step n+1 are two diagonal multiplies in the same Fourier basis, so they may be applied as ONE step of
+     * length dz (the half-steps of Eq. 15 commute with each other).  The power at node n+1 is then taken
+     * right after the nonlinear step: the closing half-step multiplies every Fourier mode by a phase times
+     * exp(-alpha_j dz/4), so P_j(z_{n+1}) = exp(-alpha_j dz/2) c_j dx dy sum |A_j|^2 (Parseval).          */
+    const int merged = (ctx->o.scheme == 0 && ctx->o.merged);
+    cplx* F1 = merged ? linear_factor(g, bm, k1, c->alpha1, c->rho1, dz) : NULL;
+    cplx* F2 = merged ? linear_factor(g, bm, k2, c->alpha2, c->rho2, dz) : NULL;
 
     double* phi  = (double*)calloc(np, sizeof(double));
     double* Tcur = (double*)malloc(sizeof(double) * np);
@@ -379,9 +387,11 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
     for (int n = 0; n < nz; ++n) {
         temperature_at_node(ctx, b, n + 1, Tnxt);
         if (ctx->o.scheme == 0) {
-            /* L/2 */
-            linear_step(A1, g, H1, brute, parallel);
-            linear_step(A2, g, H2, brute, parallel);
+            /* L/2 (merged: the opening half-step of step 0 only; later ones were applied with the previous step) */
+            if (!merged || n == 0) {
+                linear_step(A1, g, H1, brute, parallel);
+                linear_step(A2, g, H2, brute, parallel);
+            }
             /* heat source of Eq. 8, plane k <- z-step n_k = floor((2k+1) nz/(2 nq)): mean of the source
              * on the real-space fields before and after the nonlinear step (both sit at z_n + dz/2 as far as
              * the linear part goes; the mean is the trapezoid rule over the nonlinear step), G27 */
@@ -410,6 +420,15 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
             /* heat source of Eq. 8 on the planes whose sampled step is n: second half of the mean (G27) */
             if (qplane) {
                 for (size_t i = 0; i < np; ++i) qplane[i] = 0.5 * (qplane[i] + heat_source(&p, c, A1[i], A2[i]));
+            }
+            if (merged) {
+                hist[2 * (n + 1) + 0] = exp(-0.5 * c->alpha1 * dz) * grid_power(A1, np, p.c1, dxdy);
+                hist[2 * (n + 1) + 1] = exp(-0.5 * c->alpha2 * dz) * grid_power(A2, np, p.c2, dxdy);
+                /* closing half-step of step n and opening half-step of step n+1 as one step of length dz */
+                linear_step(A1, g, (n == nz - 1) ? H1 : F1, brute, parallel);
+                linear_step(A2, g, (n == nz - 1) ? H2 : F2, brute, parallel);
+                double* tt = Tcur; Tcur = Tnxt; Tnxt = tt;
+                continue;
             }
             /* L/2 */
             linear_step(A1, g, H1, brute, parallel);
@@ -446,6 +465,8 @@ static void propagate_member(orc_ctx* ctx, int b, const cplx* A1_in, const cplx*
     free(Tnxt);
     free(H1);
     free(H2);
+    free(F1);
+    free(F2);
 }
 
 int orc_propagate(orc_ctx* ctx, const double* A1_in, const double* A2_in, double* A1_out, double* A2_out,

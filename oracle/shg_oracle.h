@@ -66,6 +66,10 @@ typedef struct {
     int32_t scheme;      /* 0: L/2 - N(dz) - L/2 (north_star);  1: N/2 - L - N/2 (Eq. 14-15) */
     int32_t undepleted;  /* 1: drop the coupling term of dA1/dz ("dPump = 0")                  */
     int32_t brute_dft;   /* 1: use the O(N^2)-per-line DFT definition instead of the radix-2 FFT      */
+    int32_t merged;      /* 1 (scheme 0 only): apply the closing half-step of z-step n and the opening one of
+                            z-step n+1 as one linear step of length dz, and take P_j(z_{n+1}) right after the
+                            nonlinear step with the factor exp(-alpha_j dz/2) (Parseval) -- what a fused
+                            implementation does; pinned equal to the unmerged path at 1e-12               */
 } orc_options;
 
 int  orc_create(const orc_grid*, const orc_crystal*, const orc_beam* beams /*[batch]*/,

@@ -254,6 +254,97 @@ def test_linear_in_z_temperature_gives_quadratic_phase():
     assert np.max(np.abs(p_cold / (kappa2 ** 2 * A0 ** 4 * L * L) - 1)) < 1e-8
 
 
+def exact_phase_integral(dk_planes, L):
+    """int_0^L e^{i phi(z)} dz for a mismatch that is piecewise LINEAR in z between equidistant planes (T is linearly
+    interpolated between its planes, G15), phi(z) = int_0^z dk (Eq. 3) hence piecewise quadratic.  Independent
+    of the oracle: adaptive quadrature (scipy) interval by interval on the closed-form phase."""
+    nzt = len(dk_planes)
+    hk = L / (nzt - 1)
+    phi0 = 0.0
+    tot = 0.0 + 0.0j
+    for k in range(nzt - 1):
+        a, b = float(dk_planes[k]), float(dk_planes[k + 1])
+        ph = lambda s, a=a, b=b, phi0=phi0: phi0 + a * s + (b - a) * s * s / (2 * hk)
+        re = integrate.quad(lambda s: math.cos(ph(s)), 0.0, hk, epsabs=0.0, epsrel=1e-13)[0]
+        im = integrate.quad(lambda s: math.sin(ph(s)), 0.0, hk, epsabs=0.0, epsrel=1e-13)[0]
+        tot += re + 1j * im
+        phi0 += 0.5 * (a + b) * hk
+    return tot
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+@pytest.mark.parametrize("profile", ["linear", "planes"])
+def test_complex_sh_amplitude_pins_the_phase_samples_inside_a_step(scheme, profile):
+    """Undepleted plane wave, no absorption: A1 stays A0 and Eq. 2 reduces to the quadrature
+        A2(L) = i kappa2 A0^2 int_0^L e^{i phi(z)} dz,   phi = int_0^z dk dz'   (Eq. 3).
+    An RK4 step on a pure quadrature is Simpson's rule, so with the phase sampled where G15 puts it (z_n,
+    z_n + dz/2, z_n + dz of the in-step quadratic; scheme 1: the two half-steps of Eq. 14-15, sample at
+    0, dz/4, dz/2 and dz/2, 3dz/4, dz) the error is O(dz^4); a sample taken anywhere else is O(dz^2) or worse, and a
+    phase that does not accumulate from step to step is an O(1) error.  The COMPLEX amplitude is compared: |A2|^2
+    alone hides a mid-step phase error at first order."""
+    A0, n, nz = 3.0e3, 4, 512
+    gcoef = -40.0
+    g, c, bm, A1 = plane_wave_case(A0, nz, dk0=25.0, ddk_dT=gcoef, T_pm=0.0)
+    L = c["L"]
+    if profile == "linear":
+        nzt = 2
+        planes = np.array([0.5, 2.5])                        # T linear in z: dk from 5 to -75 rad/m
+    else:
+        nzt = 9                                              # 8 plane intervals, 64 steps each: a profile that is
+        planes = np.array([0.0, 1.75, 0.5, 2.25, 2.0, -0.75, 0.25, 1.5, 3.0])   # not linear (nor monotone) in z
+    T = np.broadcast_to(planes[:, None, None], (nzt, n, n)).astype(np.float32)   # multiples of 1/4: exact in fp32
+    expect = 1j * (2 * np.pi * c["d_eff"] / (c["n2"] * c["lambda1"])) * A0 ** 2 * \
+        exact_phase_integral(25.0 + gcoef * planes, L)
+    res = {}
+    for steps in (nz // 2, nz):
+        o = oracle.Oracle(dict(g, nz=steps, nzt=nzt), c, [bm], scheme=scheme, undepleted=True).set_temperature(T)
+        B1, B2 = o.propagate(A1)
+        assert np.max(np.abs(B1 - A0)) == 0.0                # the pump really is untouched
+        assert np.ptp(B2.real) == 0.0 and np.ptp(B2.imag) == 0.0
+        res[steps] = B2[0, 0, 0]
+    err = {k: abs(v / expect - 1) for k, v in res.items()}
+    assert err[nz] < 1e-9, err                               # measured ~1e-11
+    assert err[nz // 2] < 16 * 1.3 * max(err[nz], 1e-12) + 1e-10, err   # and it falls like dz^4
+    # guard: the quantity is sensitive -- shifting the mid-step sample by dz^2 dk'/8 (the difference between the
+    # in-step quadratic and a plain average) changes the integral by ~L dz^2 dk'/12 ~ 1e-6 relative
+    assert abs(expect) > 0.02 * (2 * np.pi * c["d_eff"] / (c["n2"] * c["lambda1"])) * A0 ** 2 * L
+
+
+def test_merged_half_steps_equal_unmerged():
+    """consecutive linear half-steps are two diagonal factors in the same Fourier basis; applying them as
+    one step of length dz (what the fused CUDA path does), with the node powers taken through Parseval, must not
+    change anything beyond rounding."""
+    w = wl.make("cfg2", nz=24)
+    res = []
+    for merged in (False, True):
+        o = oracle.Oracle(w["grid"], w["crystal"], w["beams"], merged=merged)
+        o.set_temperature(w["T"], w["T_uniform"], False)
+        a1, a2 = o.propagate(w["A1"].astype(np.complex128), 0.03j * np.roll(w["A1"], 5, axis=2).astype(np.complex128))
+        res.append((a1, a2, o.power_history()))
+    assert rel_l2(res[1][0], res[0][0]) < 1e-12 and rel_l2(res[1][1], res[0][1]) < 1e-12
+    assert np.max(np.abs(res[1][2] / res[0][2] - 1)) < 1e-12
+    assert res[0][2][-1, 1] / res[0][2][0, 0] > 1e-3         # light was converted and absorbed on the way
+    assert res[0][2][-1].sum() < res[0][2][0].sum() * (1 - 1e-3)
+
+
+def test_power_lookup_rounds_to_the_nearest_recorded_node():
+    """orc_power(z) returns the node nearest to z (P:120, P:288: powers live on the step nodes z_n = n dz);
+    checked at interior and off-node positions against exp(-alpha z_n)."""
+    c = wl.crystal(30e-3, d_eff=0.0, alpha1=7.0, alpha2=13.0)
+    bm = wl.beam(c, 2.0, 1.5, 12.0)
+    n, nz = 16, 10
+    A_in = wl.gaussian_pump(n, n, c, bm).astype(np.complex128)
+    o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=0), c, [bm])
+    o.propagate(A_in[None], 0.5j * A_in[None])
+    h = o.power_history()
+    dz = c["L"] / nz
+    for z, node in ((0.0, 0), (0.49 * dz, 0), (0.51 * dz, 1), (3.0 * dz, 3), (3.4 * dz, 3), (6.6 * dz, 7),
+                    (9.49 * dz, 9), (9.51 * dz, 10), (c["L"], 10), (1.7 * c["L"], 10), (-dz, 0)):
+        p1, p2 = o.power(0, z)
+        assert abs(p1 / (h[0, 0] * math.exp(-7.0 * node * dz)) - 1) < 1e-12, (z, node)
+        assert abs(p2 / (h[0, 1] * math.exp(-13.0 * node * dz)) - 1) < 1e-12, (z, node)
+
+
 def test_per_member_temperature_and_batch_independence():
     A0, nz, n = 1.0, 128, 4
     g, c, bm, A1 = plane_wave_case(A0, nz, ddk_dT=-30.0)
@@ -577,7 +668,8 @@ def reference_solution(c, bm, n, A1_in, A2_in, Tplanes):
             np.fft.ifft2(np.exp(lin2 * L) * y[n * n:].reshape(n, n)))
 
 
-def test_complete_path_converges_to_an_independent_solver_of_eq2():
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_complete_path_converges_to_an_independent_solver_of_eq2(scheme):
     n, nzt = 32, 6
     c = wl.crystal(8e-3, alpha=True, alpha1=3.0, alpha2=20.0, beta1=1e-11, beta2=6e-11, dk0=35.0, ddk_dT=-150.0,
                    rho1=-0.4e-3, rho2=0.9e-3)
@@ -597,7 +689,7 @@ def test_complete_path_converges_to_an_independent_solver_of_eq2():
     errs = []
     sols = []
     for nz in (40, 80, 160):                                        # plane knots sit on step nodes (5 divides nz)
-        o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=nzt), c, [bm])
+        o = oracle.Oracle(dict(nx=n, ny=n, nz=nz, nzt=nzt), c, [bm], scheme=scheme)
         o.set_temperature(T, 0.0, False)
         o1, o2 = o.propagate(A1[None], A2[None])
         sols.append((o1[0], o2[0]))
