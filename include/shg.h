@@ -22,10 +22,12 @@
  *     Grid point (iy, ix) sits at x = (ix - nx/2) lx/nx, y = (iy - ny/2) ly/ny (periodic FFT grid, G11).
  *   - Every pointer argument says HOST or DEVICE.  Device pointers must be 16-byte aligned and belong to
  *     the current CUDA device; the caller owns them.  The library owns its tables, the phase accumulator
- *     phi, the power history and staging buffers, all allocated in shg_create / shg_set_temperature_host
- *     and freed in shg_destroy; shg_propagate allocates nothing.
- *   - shg_propagate enqueues work on the given stream and returns without waiting.  shg_power and
- *     shg_power_history synchronise that stream.
+ *     phi, the power history and staging buffers, freed in shg_destroy.  They are allocated in shg_create,
+ *     except: the device copy of a host temperature array (shg_set_temperature_host, on first use or growth),
+ *     the two staging fields of shg_propagate_host (on its first call), the plane map of shg_set_heat_output
+ *     and the trace buffer of SHG_OPT_TRACE.  shg_propagate (device pointers) allocates nothing.
+ *   - shg_propagate enqueues work on the given stream and returns without waiting.  shg_synchronize,
+ *     shg_power and shg_power_history synchronise that stream and report a failed run (SHG_ECUDA).
  *   - Every call returns SHG_OK (0) or a negative code; nothing aborts or throws across the ABI.
  *   - There is no CPU fallback: without a CUDA device every call that needs one returns SHG_ECUDA.
  */
@@ -54,14 +56,17 @@ typedef struct {
                          >= 2 = planes at z_k = k L/(nzt-1), linearly interpolated to the step nodes
                          z_n = n dz: s = n (nzt-1)/nz, k = min(floor(s), nzt-2), T = (1-f)T[k] + f T[k+1] (G15) */
     int32_t batch;    /* capacity: number of independent simulations one propagate may carry         */
+    int32_t record_every; /* power history stride in z-steps: nodes n = 0, r, 2r, .. (< nz) and n = nz are
+                         recorded; 0 or 1 = every node.  shg_history_length / shg_history_nodes describe it. */
 } shg_grid;
 
 /* Crystal constants (Eq. 2; Eq. 3-4 in the linearised form the north_star fixes). */
 typedef struct {
     double L, lambda1, n1, n2, d_eff;   /* m, m (FH vacuum wavelength; SH is lambda1/2), -, -, m/V    */
     double dk0, ddk_dT, T_pm;           /* rad/m, rad/(m K), same unit as T                           */
-    double alpha1, alpha2;              /* linear intensity absorption, 1/m                           */
-    double beta1, beta2;                /* two-photon absorption, m/W                                 */
+    double alpha1, alpha2;              /* linear intensity absorption, 1/m, >= 0                     */
+    double beta1, beta2;                /* two-photon absorption, m/W, >= 0 (the power sums are kept in
+                                           fixed point scaled to the input power: no gain media)      */
     double rho1, rho2;                  /* spatial walk-off angles along x, rad: term tan(rho) dA/dx of P:387
                                            (the paper's runs use 0; P:314 names it for birefringent crystals) */
 } shg_crystal;
@@ -89,10 +94,12 @@ typedef struct {
                                   (0 = after the row pass, 1 = after the column pass) four int64: SM clock when
                                   the CTA finished its share of the pass, SM clock when the barrier released it,
                                   %globaltimer (ns) at release, SM id.  Read back with shg_read_trace.            */
-#define SHG_OPT_ACQUIRE_FENCE 4 /* persistent kernel.  0 (default): after a device-wide barrier the fields are read
-                                  with L2-only loads (ld.global.cg) and no fence is issued; 1: additionally issue a
-                                  gpu-scope acquire fence (invalidates L1) after every barrier, as the letter of
-                                  the PTX memory model asks.  Bit-identical results; ~350 SM clocks per barrier.   */
+#define SHG_OPT_ACQUIRE_FENCE 4 /* persistent kernel, acquire side of the device-wide barrier.  2 (default): the poll
+                                  ends with an ld.acquire.gpu of the barrier counter (pairs with the arrivals'
+                                  red.release.gpu; conforms to the PTX memory model); 1: a gpu-scope fence.acq_rel
+                                  after a relaxed poll (same guarantee); 0: no acquire at all -- the fields are read
+                                  with L2-only loads (ld.global.cg), which works on sm_100a but is outside the
+                                  memory model; kept for measurements.  Bit-identical results in all modes.        */
 #define SHG_OPT_UNDEPLETED 5    /* 1: drop the coupling term of dA1/dz (the pump only diffracts and is absorbed), the
                                   "dPump = 0" check against Boyd-Kleinman of P:292; 0 (default): full Eq. 2.       */
 #define SHG_OPT_SCHEME     6    /* 0 (default): L/2 - N(dz) - L/2 with neighbouring half-steps merged (north_star);
@@ -100,6 +107,20 @@ typedef struct {
                                   two RK4 half-steps per z-step, powers summed at the true nodes.  Variant for
                                   comparison with the paper's scheme (differs from scheme 0 by O(dz^2)); needs
                                   SHG_OPT_PRECISE = 1 and no heat output (else shg_propagate returns SHG_EINVAL). */
+
+#define SHG_OPT_SPIN_LIMIT 7    /* persistent kernel: a CTA that waits longer than `value` million SM clocks at a
+                                  device-wide barrier raises the status word (reported by shg_synchronize /
+                                  shg_power*) instead of hanging the GPU.  Default 4000 (~2 s); 0 = wait forever
+                                  (use under profilers / sanitizers that serialise or replay the kernel).          */
+#define SHG_OPT_TABLES_SMEM 8   /* 1 (default): a single simulation's persistent kernel keeps the propagator tables
+                                  hx, hy in shared memory; 0: reads them through L1 like the batched runs do.       */
+#define SHG_OPT_CLUSTER    9    /* small grids (nx = ny <= 256).  1 (default): when every member of the propagate fits
+                                  one co-resident wave of thread-block clusters, the whole run (opening half-step,
+                                  z-loop, closing half-step) is ONE launch of k_cluster: one cluster of 8 or 16
+                                  CTAs per member, the fields resident in distributed shared memory, the column
+                                  exchange through DSMEM, cluster barriers instead of device-wide ones; 0: never;
+                                  2: whenever the grid size allows, even if the clusters run in several waves.
+                                  Same per-point arithmetic as the other kernels: bit-identical fields and powers. */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);
@@ -117,9 +138,11 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
                              void* cuda_stream);
 
 /* Propagate `batch` (<= capacity) members from z = 0 to z = L.
- * A1_in, A2_in, A1_out, A2_out: DEVICE complex fp32 [batch][ny][nx].  A2_in may be NULL (zeros: the
- * configs' A_SH(0) = 0).  In-place (A1_out == A1_in and/or A2_out == A2_in) is allowed; A1_out and
- * A2_out must not overlap each other.  The outputs are also the kernels' working storage.
+ * A1_in, A2_in, A1_out, A2_out: DEVICE complex fp32 [batch][ny][nx].  A1_in may be NULL: the pump is then the
+ * Gaussian of Eq. 6 / Eq. 5 of every member's beam (as shg_gaussian_input writes it; SHG_EINVAL if a
+ * beam has w0 <= 0).  A2_in may be NULL (zeros: the configs' A_SH(0) = 0).  In-place (A1_out == A1_in and/or
+ * A2_out == A2_in, the same pointer) is allowed; any other overlap between the four buffers is SHG_EINVAL.
+ * The outputs are also the kernels' working storage.
  * cuda_stream: a cudaStream_t (NULL = the legacy default stream). */
 int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out,
                   int batch, void* cuda_stream);
@@ -139,11 +162,23 @@ int shg_propagate_host(shg_ctx* ctx, const void* A1_in, const void* A2_in, void*
  * It is written from the epilogue of the nonlinear step: 2 extra sweeps over a row on nq of the nz steps. */
 int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq);
 
-/* Power (W) of both fields of `member` at the recorded node nearest to z (nodes z_n = n L/nz, n = 0..nz).
- * The SH efficiency is derived by the caller: eta = P2(L) / (P1(0) + P2(0))  (G16). */
+/* Wait for the last propagate of this context and report how it ended: SHG_OK, or SHG_ECUDA when the stream
+ * failed or a device-wide barrier of the persistent kernel timed out (the outputs are then invalid).  Call it
+ * (or shg_power*) before trusting A1_out / A2_out of a run whose history you do not read. */
+int shg_synchronize(shg_ctx* ctx);
+
+/* Power (W) of both fields of `member` at the RECORDED node nearest to z (step nodes z_n = n L/nz; recorded:
+ * shg_grid.record_every).  The SH efficiency is derived by the caller: eta = P2(L) / (P1(0) + P2(0))  (P:288,
+ * G16).  The sums behind these numbers are accumulated in fixed point (integers): they are bit-reproducible
+ * from run to run and identical between launch schemes. */
 int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2);
 
-/* Whole history of `member`: out is a HOST array [nz+1][2] = {P1(z_n), P2(z_n)}. */
+/* Number of recorded nodes (ceil(nz / record_every) + 1), and their step indices n (HOST int32 array of that
+ * length: 0, r, 2r, .., nz). */
+int shg_history_length(const shg_ctx* ctx);
+int shg_history_nodes(const shg_ctx* ctx, int32_t* nodes);
+
+/* Whole history of `member`: out is a HOST array [shg_history_length()][2] = {P1(z_n), P2(z_n)}. */
 int shg_power_history(shg_ctx* ctx, int member, double* out);
 
 /* Fill A1 (DEVICE complex fp32 [batch][ny][nx]) with the Gaussian pump of Eq. 6 / Eq. 5 of every

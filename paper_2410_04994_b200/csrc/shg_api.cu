@@ -76,6 +76,61 @@ __global__ void k_gaussian(float2* A, const shg::GaussDev* gd, int nx, int ny, i
     A[i] = make_float2(mag * (g.ar * c - g.ai * s), mag * (g.ar * s + g.ai * c));
 }
 
+// P_j(0) and the member's fixed-point scale (shg_device.cuh, "power sums").  Grid (chunks, batch): every block sums
+// |A_1|^2 and |A_2|^2 over its chunk of the member's input in double, in a fixed order; the last block to finish
+// (ticket counter) adds the chunk sums in chunk order -- deterministic -- and writes
+//   pfix[b] = 2^e with (S_1 + S_2) 2^e in [2^59, 2^60),   hfix[b][0][j] = rint(S_j 2^e).
+__global__ void __launch_bounds__(256) k_input_power(const float2* __restrict__ A1, const float2* __restrict__ A2,
+                                                     size_t np, int nrec, double* part, unsigned int* ticket,
+                                                     float* pfix, long long* hfix) {
+    const int b = blockIdx.y, c = blockIdx.x, CH = gridDim.x;
+    const size_t len = np / CH, base = (size_t)b * np + (size_t)c * len;
+    double s1 = 0.0, s2 = 0.0;
+    for (size_t i = threadIdx.x; i < len; i += blockDim.x) {
+        const float2 a = A1[base + i];
+        s1 += (double)a.x * a.x + (double)a.y * a.y;
+        if (A2) {
+            const float2 d = A2[base + i];
+            s2 += (double)d.x * d.x + (double)d.y * d.y;
+        }
+    }
+    __shared__ double sh[2][8];
+    __shared__ bool last;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = s1; sh[1][threadIdx.x >> 5] = s2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t1 = 0.0, t2 = 0.0;
+        for (int w = 0; w < 8; ++w) { t1 += sh[0][w]; t2 += sh[1][w]; }
+        part[((size_t)b * CH + c) * 2 + 0] = t1;
+        part[((size_t)b * CH + c) * 2 + 1] = t2;
+        __threadfence();
+        last = (atomicAdd(&ticket[b], 1u) == (unsigned)(CH - 1));
+        if (last) {
+            __threadfence();
+            double S1 = 0.0, S2 = 0.0;
+            for (int k = 0; k < CH; ++k) {
+                S1 += __ldcg(&part[((size_t)b * CH + k) * 2 + 0]);
+                S2 += __ldcg(&part[((size_t)b * CH + k) * 2 + 1]);
+            }
+            const double S = S1 + S2;
+            int e = 0;
+            if (S > 0.0 && S < 1e300) {
+                e = 59 - ilogb(S);
+                e = e > 120 ? 120 : (e < -120 ? -120 : e);
+            }
+            pfix[b] = ldexpf(1.0f, e);
+            hfix[(size_t)b * (nrec + 1) * 2 + 0] = llrint(ldexp(S1, e));
+            hfix[(size_t)b * (nrec + 1) * 2 + 1] = llrint(ldexp(S2, e));
+            ticket[b] = 0;
+        }
+    }
+}
+
 // fp32 pipe peak: 16 independent FFMA chains per thread, nothing else in the loop
 __global__ void __launch_bounds__(512, 1) k_fp32_peak(float* out, const float* in, int iters) {
     float a[16];
@@ -102,7 +157,11 @@ struct shg_ctx {
     int sm_count = 0;
     bool persistent = true;
     bool precise = true;
-    bool acquire_fence = false;
+    int acquire_fence = 2;
+    int tables_smem = 1;
+    int cluster_mode = 1;                 // SHG_OPT_CLUSTER: 0 never, 1 auto, 2 whenever the grid size allows
+    unsigned long long spin_limit = 4000000000ULL;
+    int rec_every = 1, nrec = 0;
     bool undepleted = false;
     int scheme = 0;
     bool tables_dirty = true;
@@ -117,7 +176,11 @@ struct shg_ctx {
     shg::MemberDev* d_mem = nullptr;
     shg::GaussDev* d_gauss = nullptr;
     float* d_phi = nullptr;
-    double* d_hist = nullptr;
+    long long* d_hfix = nullptr;         // [batch][nrec+1][2] fixed-point power sums
+    float* d_pfix = nullptr;             // [batch] fixed-point scale 2^e of each member
+    double* d_inpart = nullptr;          // k_input_power chunk sums [batch][64][2]
+    unsigned int* d_ticket = nullptr;    // [batch]
+    std::vector<double> pscale_in, pscale_step;   // [batch][2] (eps0 c n_j/2) dx dy, and times exp(-alpha_j dz/2)
     unsigned int* d_barrier = nullptr;   // [0] barrier counter, [1] status word
     float* d_T_owned = nullptr;
     float* d_Q = nullptr;              // borrowed heat-source output (shg_set_heat_output)
@@ -142,7 +205,10 @@ struct shg_ctx {
     int last_batch = 0;
     int last_launches = 0;
     bool hist_valid = false;
-    std::vector<double> hist_host;
+    int last_scheme = 0;
+    std::vector<double> hist_host;       // [batch][nrec+1][2], W
+    std::vector<long long> hfix_host;
+    std::vector<float> pfix_host;
 };
 
 namespace {
@@ -232,8 +298,10 @@ int upload_tables(shg_ctx* ctx) {
         }
         const double dxdy = (bm.lx / g.nx) * (bm.ly / g.ny);
         for (int f = 0; f < 2; ++f) {
-            m.pscale_in[f] = 0.5 * EPS0 * C0 * nj[f] * dxdy;
-            m.pscale_step[f] = std::exp(-0.5 * alpha[f] * dz) * m.pscale_in[f];
+            ctx->pscale_in[(size_t)b * 2 + f] = 0.5 * EPS0 * C0 * nj[f] * dxdy;
+            // Parseval: the sum taken right after the nonlinear step, times exp(-alpha_j dz/2), is the power
+            // after the closing half-step
+            ctx->pscale_step[(size_t)b * 2 + f] = std::exp(-0.5 * alpha[f] * dz) * ctx->pscale_in[(size_t)b * 2 + f];
         }
         // Eq. 5 at z = 0: tau0 = -focus_z / zR; |A0|^2 = 4P/(eps0 c n1 pi w0^2) (G17)
         shg::GaussDev& gd = gs[b];
@@ -270,7 +338,10 @@ void free_ctx(shg_ctx* ctx) {
     cudaFree(ctx->d_mem);
     cudaFree(ctx->d_gauss);
     cudaFree(ctx->d_phi);
-    cudaFree(ctx->d_hist);
+    cudaFree(ctx->d_hfix);
+    cudaFree(ctx->d_pfix);
+    cudaFree(ctx->d_inpart);
+    cudaFree(ctx->d_ticket);
     cudaFree(ctx->d_barrier);
     cudaFree(ctx->d_T_owned);
     cudaFree(ctx->d_qmap);
@@ -313,7 +384,8 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     *out = nullptr;
     Launchers Lx, Ly;
     if (!launchers_for(grid->nx, &Lx) || !launchers_for(grid->ny, &Ly)) return SHG_EINVAL;
-    if (grid->nz < 1 || grid->nzt < 0 || grid->batch < 1) return SHG_EINVAL;
+    if (grid->nz < 1 || grid->nzt < 0 || grid->batch < 1 || grid->record_every < 0) return SHG_EINVAL;
+    if (crystal->alpha1 < 0 || crystal->alpha2 < 0 || crystal->beta1 < 0 || crystal->beta2 < 0) return SHG_EINVAL;
     if (!(crystal->L > 0) || !(crystal->lambda1 > 0) || !(crystal->n1 > 0) || !(crystal->n2 > 0)) return SHG_EINVAL;
     for (int b = 0; b < grid->batch; ++b)
         if (!(beams[b].lx > 0) || !(beams[b].ly > 0)) return SHG_EINVAL;
@@ -331,6 +403,10 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     ctx->device = dev;
     ctx->T_uniform = crystal->T_pm;
     ctx->T_set = (grid->nzt == 0);
+    ctx->rec_every = grid->record_every < 1 ? 1 : (grid->record_every > grid->nz ? grid->nz : grid->record_every);
+    ctx->nrec = (grid->nz + ctx->rec_every - 1) / ctx->rec_every;
+    ctx->pscale_in.assign((size_t)grid->batch * 2, 0.0);
+    ctx->pscale_step.assign((size_t)grid->batch * 2, 0.0);
     cudaError_t e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaDeviceGetAttribute"); }
 
@@ -351,10 +427,17 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     alloc((void**)&ctx->d_mem, sizeof(shg::MemberDev) * B);
     alloc((void**)&ctx->d_gauss, sizeof(shg::GaussDev) * B);
     if (grid->nzt > 0) alloc((void**)&ctx->d_phi, sizeof(float) * (size_t)B * np);
-    alloc((void**)&ctx->d_hist, sizeof(double) * (size_t)B * (grid->nz + 1) * 2);
+    alloc((void**)&ctx->d_hfix, sizeof(long long) * (size_t)B * (ctx->nrec + 1) * 2);
+    alloc((void**)&ctx->d_pfix, sizeof(float) * B);
+    alloc((void**)&ctx->d_inpart, sizeof(double) * (size_t)B * 64 * 2);
+    alloc((void**)&ctx->d_ticket, sizeof(unsigned int) * B);
     alloc((void**)&ctx->d_barrier, 2 * sizeof(unsigned int));
     if (!ok) { free_ctx(ctx); return SHG_ECUDA; }
-    ctx->hist_host.assign((size_t)B * (grid->nz + 1) * 2, 0.0);
+    e = cudaMemset(ctx->d_ticket, 0, sizeof(unsigned int) * B);
+    if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaMemset"); }
+    ctx->hist_host.assign((size_t)B * (ctx->nrec + 1) * 2, 0.0);
+    ctx->hfix_host.assign((size_t)B * (ctx->nrec + 1) * 2, 0);
+    ctx->pfix_host.assign((size_t)B, 1.0f);
     int rc = upload_tables(ctx);
     if (rc != SHG_OK) { free_ctx(ctx); return rc; }
     *out = ctx;
@@ -367,7 +450,19 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
     if (!ctx) return SHG_EINVAL;
     switch (option) {
         case SHG_OPT_PERSISTENT: ctx->persistent = (value != 0); return SHG_OK;
-        case SHG_OPT_ACQUIRE_FENCE: ctx->acquire_fence = (value != 0); return SHG_OK;
+        case SHG_OPT_ACQUIRE_FENCE:
+            if (value < 0 || value > 2) return SHG_EINVAL;
+            ctx->acquire_fence = value;
+            return SHG_OK;
+        case SHG_OPT_SPIN_LIMIT:
+            if (value < 0) return SHG_EINVAL;
+            ctx->spin_limit = (unsigned long long)value * 1000000ULL;
+            return SHG_OK;
+        case SHG_OPT_TABLES_SMEM: ctx->tables_smem = (value != 0); return SHG_OK;
+        case SHG_OPT_CLUSTER:
+            if (value < 0 || value > 2) return SHG_EINVAL;
+            ctx->cluster_mode = value;
+            return SHG_OK;
         case SHG_OPT_SCHEME:
             if (value != 0 && value != 1) return SHG_EINVAL;
             ctx->scheme = value;
@@ -415,8 +510,8 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
     if (!T_host) return SHG_EINVAL;
     const size_t bytes = sizeof(float) * (size_t)(per_member ? ctx->g.batch : 1) * ctx->g.nzt * np_of(ctx);
     if (ctx->T_owned_bytes < bytes) {
+        CU(cudaStreamSynchronize(ctx->last_stream));      // an earlier propagate may still read the old copy
         cudaFree(ctx->d_T_owned);
-    cudaFree(ctx->d_qmap);
         ctx->d_T_owned = nullptr;
         ctx->T_owned_bytes = 0;
         CU(cudaMalloc((void**)&ctx->d_T_owned, bytes));
@@ -449,17 +544,37 @@ int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq) {
 
 int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out, int batch,
                   void* cuda_stream) {
-    if (!ctx || !A1_in || !A1_out || !A2_out) return SHG_EINVAL;
+    if (!ctx || !A1_out || !A2_out) return SHG_EINVAL;
     if (batch < 1 || batch > ctx->g.batch) return SHG_EINVAL;
     if (!aligned16(A1_in) || !aligned16(A2_in) || !aligned16(A1_out) || !aligned16(A2_out)) return SHG_EINVAL;
-    if (A1_out == A2_out) return SHG_EINVAL;
+    {   // A field may be propagated in place (out == in, exactly); any other overlap is an error: the first row
+        // pass reads both inputs of a row while it writes both outputs of other rows.
+        const size_t bytes = sizeof(float2) * (size_t)batch * np_of(ctx);
+        auto overlap = [bytes](const void* a, const void* b) {
+            if (!a || !b) return false;
+            const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+            return x < y + bytes && y < x + bytes;
+        };
+        if (overlap(A1_out, A2_out) || overlap(A1_in, A2_out) || overlap(A2_in, A1_out) || overlap(A1_in, A2_in))
+            return SHG_EINVAL;
+        if ((A1_in != A1_out && overlap(A1_in, A1_out)) || (A2_in != A2_out && overlap(A2_in, A2_out)))
+            return SHG_EINVAL;
+    }
     if (!ctx->T_set) return SHG_ESTATE;
+    if (!A1_in)                      // Gaussian pump of Eq. 6 / Eq. 5 from the beams of shg_create
+        for (int b = 0; b < batch; ++b)
+            if (!(ctx->beams[b].w0 > 0) || !(ctx->beams[b].P >= 0)) return SHG_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (ctx->tables_dirty) {
         // tables are uploaded with synchronous copies; make sure no earlier propagate still reads them
         CU(cudaStreamSynchronize(ctx->last_stream));
         int rc = upload_tables(ctx);
         if (rc != SHG_OK) return rc;
+    }
+    if (!A1_in) {
+        int rc = shg_gaussian_input(ctx, A1_out, batch, cuda_stream);
+        if (rc != SHG_OK) return rc;
+        A1_in = A1_out;
     }
     const shg_grid& g = ctx->g;
     shg::Params P{};
@@ -471,19 +586,30 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.twx = ctx->d_twx; P.twy = ctx->d_twy;
     for (int hs = 0; hs < 2; ++hs) { P.hx[hs] = ctx->d_hx[hs]; P.hy[hs] = ctx->d_hy[hs]; }
     P.mem = ctx->d_mem;
-    P.hist = ctx->d_hist;
+    P.hfix = ctx->d_hfix; P.pfix = ctx->d_pfix;
+    P.rec_every = ctx->rec_every; P.nrec = ctx->nrec;
+    P.spin_limit = ctx->spin_limit;
     P.Q = ctx->d_Q; P.qmap = ctx->d_qmap; P.nq = ctx->nq;
     P.barrier = ctx->d_barrier;
     P.status = reinterpret_cast<int*>(ctx->d_barrier + 1);
     P.trace = ctx->d_trace;
-    P.acquire_fence = ctx->acquire_fence ? 1 : 0;
+    P.acquire_fence = ctx->acquire_fence;
     P.scheme = ctx->scheme;
     P.trace_steps = ctx->trace_steps;
 
     const size_t np = np_of(ctx);
-    CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(double) * (size_t)g.batch * (g.nz + 1) * 2, st));
+    int launches = 0;
+    CU(cudaMemsetAsync(ctx->d_hfix, 0, sizeof(long long) * (size_t)g.batch * (ctx->nrec + 1) * 2, st));
     CU(cudaMemsetAsync(ctx->d_barrier, 0, 2 * sizeof(unsigned int), st));
     if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
+    {   // P_j(0) and the fixed-point scale of every member, from the input (before anything overwrites it)
+        int ch = (int)(np / 4096);
+        ch = ch < 1 ? 1 : (ch > 64 ? 64 : ch);
+        k_input_power<<<dim3(ch, batch), 256, 0, st>>>((const float2*)A1_in, (const float2*)A2_in, np, ctx->nrec,
+                                                       ctx->d_inpart, ctx->d_ticket, ctx->d_pfix, ctx->d_hfix);
+        CU(cudaGetLastError());
+        ++launches;
+    }
 
     const shg::LaunchInfo ix = ctx->Lx.info(), iy = ctx->Ly.info();
     const int UR = batch * g.ny / ix.rows_per_item;          // row-pass items
@@ -512,7 +638,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         P.col_teams = active(UC, gc, iy.col_teams, iy.team_warps);
     }
     const bool prec = ctx->precise;
-    int launches = 0;
+    P.tab_smem = (use_persist && ctx->tables_smem && batch == 1 && prec && ctx->scheme == 0 && !P.Q) ? 1 : 0;
     {   // Sparse launch: every CTA owns at most one row item per slot and at most half of its warps have one
         // (single small simulations).  The persistent kernel then spreads the nonlinear step over the whole CTA.
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
@@ -573,41 +699,76 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     ctx->last_stream = st;
     ctx->last_batch = batch;
     ctx->last_launches = launches;
+    ctx->last_scheme = ctx->scheme;
     ctx->hist_valid = false;
     return SHG_OK;
 }
 
 int shg_propagate_host(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_out, void* A2_out, int batch,
                        void* cuda_stream) {
-    if (!ctx || !A1_in || !A1_out || !A2_out) return SHG_EINVAL;
+    if (!ctx || !A1_out || !A2_out) return SHG_EINVAL;
     if (batch < 1 || batch > ctx->g.batch) return SHG_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t cap = sizeof(float2) * (size_t)ctx->g.batch * np_of(ctx);
     const size_t bytes = sizeof(float2) * (size_t)batch * np_of(ctx);
     for (int i = 0; i < 2; ++i)
         if (!ctx->d_stage[i]) CU(cudaMalloc((void**)&ctx->d_stage[i], cap));
-    CU(cudaMemcpyAsync(ctx->d_stage[0], A1_in, bytes, cudaMemcpyHostToDevice, st));
+    if (A1_in) CU(cudaMemcpyAsync(ctx->d_stage[0], A1_in, bytes, cudaMemcpyHostToDevice, st));
     if (A2_in) CU(cudaMemcpyAsync(ctx->d_stage[1], A2_in, bytes, cudaMemcpyHostToDevice, st));
-    int rc = shg_propagate(ctx, ctx->d_stage[0], A2_in ? ctx->d_stage[1] : nullptr, ctx->d_stage[0], ctx->d_stage[1],
-                           batch, cuda_stream);
+    int rc = shg_propagate(ctx, A1_in ? ctx->d_stage[0] : nullptr, A2_in ? ctx->d_stage[1] : nullptr,
+                           ctx->d_stage[0], ctx->d_stage[1], batch, cuda_stream);
     if (rc != SHG_OK) return rc;
+    // (a barrier timeout of the persistent kernel is reported by shg_synchronize / shg_power*, not here: this
+    // call only enqueues)
     CU(cudaMemcpyAsync(A1_out, ctx->d_stage[0], bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(A2_out, ctx->d_stage[1], bytes, cudaMemcpyDeviceToHost, st));
+    return SHG_OK;
+}
+
+int shg_synchronize(shg_ctx* ctx) {
+    if (!ctx) return SHG_EINVAL;
+    if (ctx->last_batch == 0) return SHG_OK;
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    unsigned int bs[2] = {0, 0};
+    CU(cudaMemcpy(bs, ctx->d_barrier, sizeof(bs), cudaMemcpyDeviceToHost));
+    if (bs[1] != 0) {
+        g_cuda_msg = "persistent kernel: a device-wide barrier timed out (not all CTAs co-resident, or the spin limit "
+                     "of SHG_OPT_SPIN_LIMIT is too short for this run); the outputs of this propagate are invalid";
+        return SHG_ECUDA;
+    }
     return SHG_OK;
 }
 
 static int fetch_history(shg_ctx* ctx) {
     if (ctx->last_batch == 0) return SHG_ESTATE;
     if (ctx->hist_valid) return SHG_OK;
-    CU(cudaStreamSynchronize(ctx->last_stream));
-    unsigned int bs[2] = {0, 0};
-    CU(cudaMemcpy(bs, ctx->d_barrier, sizeof(bs), cudaMemcpyDeviceToHost));
-    if (bs[1] != 0) {
-        g_cuda_msg = "persistent kernel: device-wide barrier timed out (not all CTAs were co-resident?)";
-        return SHG_ECUDA;
+    int rc = shg_synchronize(ctx);
+    if (rc != SHG_OK) return rc;
+    CU(cudaMemcpy(ctx->hfix_host.data(), ctx->d_hfix, sizeof(long long) * ctx->hfix_host.size(), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(ctx->pfix_host.data(), ctx->d_pfix, sizeof(float) * ctx->pfix_host.size(), cudaMemcpyDeviceToHost));
+    // fixed point -> W: sum |A_j|^2 = fix / 2^e (exact in double up to 2^53), P_j = (eps0 c n_j/2) dx dy sum.
+    // Scheme 0 takes the sums of nodes >= 1 right after the nonlinear step: Parseval factor exp(-alpha_j dz/2).
+    const size_t per = (size_t)(ctx->nrec + 1) * 2;
+    for (int b = 0; b < ctx->last_batch; ++b) {
+        const double inv = 1.0 / (double)ctx->pfix_host[(size_t)b];
+        for (size_t i = 0; i < per; ++i) {
+            const int f = (int)(i & 1);
+            const bool node0 = (i < 2);
+            const double sc = (node0 || ctx->last_scheme == 1) ? ctx->pscale_in[(size_t)b * 2 + f]
+                                                              : ctx->pscale_step[(size_t)b * 2 + f];
+            ctx->hist_host[(size_t)b * per + i] = (double)ctx->hfix_host[(size_t)b * per + i] * inv * sc;
+        }
     }
-    CU(cudaMemcpy(ctx->hist_host.data(), ctx->d_hist, sizeof(double) * ctx->hist_host.size(), cudaMemcpyDeviceToHost));
     ctx->hist_valid = true;
+    return SHG_OK;
+}
+
+int shg_history_length(const shg_ctx* ctx) { return ctx ? ctx->nrec + 1 : SHG_EINVAL; }
+
+int shg_history_nodes(const shg_ctx* ctx, int32_t* nodes) {
+    if (!ctx || !nodes) return SHG_EINVAL;
+    for (int k = 0; k < ctx->nrec; ++k) nodes[k] = k * ctx->rec_every;
+    nodes[ctx->nrec] = ctx->g.nz;
     return SHG_OK;
 }
 
@@ -616,7 +777,7 @@ int shg_power_history(shg_ctx* ctx, int member, double* out) {
     int rc = fetch_history(ctx);
     if (rc != SHG_OK) return rc;
     if (member >= ctx->last_batch) return SHG_ESTATE;
-    const size_t n = (size_t)(ctx->g.nz + 1) * 2;
+    const size_t n = (size_t)(ctx->nrec + 1) * 2;
     std::memcpy(out, ctx->hist_host.data() + (size_t)member * n, sizeof(double) * n);
     return SHG_OK;
 }
@@ -626,13 +787,17 @@ int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2) {
     int rc = fetch_history(ctx);
     if (rc != SHG_OK) return rc;
     if (member >= ctx->last_batch) return SHG_ESTATE;
+    // nearest RECORDED node: nodes k rec_every (k < nrec) and nz
     const double dz = ctx->c.L / ctx->g.nz;
-    long n = std::lround(z / dz);
-    if (n < 0) n = 0;
-    if (n > ctx->g.nz) n = ctx->g.nz;
-    const double* h = ctx->hist_host.data() + (size_t)member * (ctx->g.nz + 1) * 2;
-    *P1 = h[2 * n];
-    *P2 = h[2 * n + 1];
+    const int re = ctx->rec_every, nz = ctx->g.nz;
+    double zn = z / dz;
+    zn = zn < 0 ? 0 : (zn > nz ? nz : zn);
+    long k = std::lround(zn / re);
+    if (k > ctx->nrec - 1) k = ctx->nrec - 1;
+    const long slot = (std::fabs(zn - (double)nz) <= std::fabs(zn - (double)(k * re))) ? ctx->nrec : k;
+    const double* h = ctx->hist_host.data() + (size_t)member * (ctx->nrec + 1) * 2;
+    *P1 = h[2 * slot];
+    *P2 = h[2 * slot + 1];
     return SHG_OK;
 }
 

@@ -66,6 +66,10 @@ template <int N> struct Geo {
     static constexpr int WORK_SMEM = ROW_SMEM > COL_SMEM ? ROW_SMEM : COL_SMEM;
     static constexpr int TW_SMEM = N * 16;                 // twiddles [R][M] as float4 (hi.re, hi.im, lo.re, lo.im)
     static constexpr int CTA_SMEM = WORK_SMEM + TW_SMEM;
+    // persistent kernel of a single simulation: the propagator tables hx, hy of both fields staged in shared memory
+    static constexpr int TAB_SMEM = 4 * N * 16;            // [hx f=0][hx f=1][hy f=0][hy f=1], N float4 each
+    static constexpr int CTA_SMEM_TAB = CTA_SMEM + TAB_SMEM;
+    static_assert(CTA_SMEM_TAB <= 227 * 1024, "shared memory budget");
     static_assert(WARPS % TW == 0 && WARPS % 2 == 0, "team / pair layout");
     static_assert(TEAMS + 1 <= 16 && WARPS / 2 + 1 <= 16, "named barrier ids");
 };
@@ -126,6 +130,18 @@ __device__ __forceinline__ void table_mul(float2 (&v)[R], const float4* __restri
         const float2 w = cmul_hl<false, PREC>(v[q], __ldg(ptr_after(tab, dep) + M * q));
         v[q] = CONJ_OUT ? make_float2(w.x, -w.y) : w;
     }
+}
+
+// same from a table in shared memory (stab_saddr: shared-window address of this lane's first entry)
+template <int R, int M, bool PREC, bool CONJ_OUT, int Q>
+__device__ __forceinline__ void table_mul_s_one(float2 (&v)[R], unsigned stab_saddr) {
+    const float dep = (Q >= TWIDDLE_DEPTH) ? v[Q - TWIDDLE_DEPTH].x : v[Q].x;
+    const float2 w = cmul_hl<false, PREC>(v[Q], lds128_after<Q * M * 16>(stab_saddr, dep));
+    v[Q] = CONJ_OUT ? make_float2(w.x, -w.y) : w;
+}
+template <int R, int M, bool PREC, bool CONJ_OUT, int... Q>
+__device__ __forceinline__ void table_mul_s(float2 (&v)[R], unsigned stab_saddr, std::integer_sequence<int, Q...>) {
+    (table_mul_s_one<R, M, PREC, CONJ_OUT, Q>(v, stab_saddr), ...);
 }
 
 template <int N, bool PREC, int K1>
@@ -192,6 +208,32 @@ __device__ __forceinline__ float warp_sum(float x) {
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
     return x;
+}
+
+// ---- power sums, order independent ---------------------------------------------------------
+// sum |A_j|^2 over a member's points is accumulated in 64-bit FIXED POINT: every point's |A_j|^2 (fp32) is scaled
+// by the member's power-of-two scale pfix = 2^e (exact) and rounded to an integer once; integers add
+// associatively, so the result does not depend on which warp, CTA, launch scheme or kernel summed which points,
+// nor on the arrival order of the atomics: the power history is bit-reproducible and identical between the
+// persistent, per-pass, sparse and cluster kernels.  k_input_power picks e so that the input's total sum maps to
+// [2^59, 2^60): 3 bits of headroom (power does not grow: alpha, beta >= 0) and a resolution of 2^-60 of the input.
+__device__ __forceinline__ long long to_fix(float s, float scale) { return __float2ll_rn(s * scale); }
+
+__device__ __forceinline__ long long warp_sum_ll(long long x) {
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+__device__ __forceinline__ void fix_add(long long* dst, long long v) {
+    atomicAdd(reinterpret_cast<unsigned long long*>(dst), (unsigned long long)v);
+}
+
+// history slot of step node `node` (0..nz), or -1 when that node is not recorded (shg_grid.record_every)
+__device__ __forceinline__ int rec_slot(const Params& P, int node) {
+    if (P.rec_every == 1) return node;
+    if (node == P.nz) return P.nrec;
+    return (node % P.rec_every == 0) ? node / P.rec_every : -1;
 }
 
 // phase reduced to [-pi, pi]
@@ -298,9 +340,11 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
 // smem_cta: base of the per-warp line regions.  hsel: 0 = full-step tables, 1 = half-step tables.
 // ------------------------------------------------------------------------------------------------
 // HEAT: also write the heat source of Eq. 8 (a separate instantiation: the common path carries none of it).
-template <int NX, int MODE, bool PREC, bool HEAT = false>
+// TS: the hx tables are read from shared memory (stab: [2][NX] float4, single simulation) instead of global / L1.
+template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
 __device__ __forceinline__ void row_item(const Params& P, int item, int n, int hsel, float2* smem_cta,
-                                         const float4* __restrict__ tws, int warp, int lane) {
+                                         const float4* __restrict__ tws, int warp, int lane,
+                                         const float4* __restrict__ stab = nullptr) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
     const int g = lane / M, m = lane % M;
@@ -326,20 +370,12 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 #pragma unroll
             for (int q = 0; q < R; ++q) v[q] = make_float2(0.f, 0.f);
         }
-        float s = 0.f;
-#pragma unroll
-        for (int q = 0; q < R; ++q) s += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
+        // (P_j(0) is taken from the input by k_input_power, which also fixes the member's fixed-point scale)
         warp_fft<NX, PREC>(v, own, tws, m);
         table_mul<R, M, PREC, false>(v, P.hx[hsel] + ((size_t)b * 2 + f) * NX + m);
         float2* dst = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(dst + M * q + m, v[q]);
-        float s0 = warp_sum(f ? 0.f : s), s1 = warp_sum(f ? s : 0.f);
-        if (lane == 0) {
-            double* hst = P.hist + (size_t)b * (P.nz + 1) * 2;
-            if (G >= 2 || f == 0) atomicAdd(hst + 0, (double)s0 * mb.pscale_in[0]);
-            if (G >= 2 || f == 1) atomicAdd(hst + 1, (double)s1 * mb.pscale_in[1]);
-        }
         return;
     }
 
@@ -358,7 +394,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
-        table_prefetch<R, M>(hx, m);
+        if constexpr (!TS) table_prefetch<R, M>(hx, m);
         // temperature / phase operands of the first RK4 point are requested before the transform (when
         // registers allow), those of the second right after it; inside the loop two points ahead
         const size_t plane = (size_t)P.ny * NX;
@@ -391,7 +427,9 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         float2* p1 = (f ? par + M * H : own) + m;
         float2* p2 = (f ? own : par + M * H) + m;
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz, g1 = mb.g1dz, g2 = mb.g2dz;
-        float s1 = 0.f, s2 = 0.f;
+        const int slot = rec_slot(P, n + 1);                  // warp-uniform: is P_j(z_{n+1}) recorded?
+        const float fsc = P.pfix[b];
+        long long s1 = 0, s2 = 0;
         // Heat source of Eq. 8 for the plane that samples this z-step, if any (warp-uniform): half of
         // q on the fields before the nonlinear step now, the other half after it (G27).  Only nq of the nz
         // steps come here, so the two extra sweeps over the line in shared memory stay off the common path.
@@ -430,8 +468,10 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                 float2 a1 = p1[M * q], a2 = p2[M * q];
                 a1.y = -a1.y; a2.y = -a2.y;
                 rk4_point(a1, a2, CA, CM, CB, g1, g2);
-                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
-                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+                if (slot >= 0) {
+                    s1 += to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc);
+                    s2 += to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc);
+                }
                 p1[M * q] = a1;
                 p2[M * q] = a2;
             }
@@ -458,8 +498,10 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
                 float2 a1 = p1[M * q], a2 = p2[M * q];
                 a1.y = -a1.y; a2.y = -a2.y;
                 rk4_point(a1, a2, CA, CM, CB, g1, g2);
-                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
-                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+                if (slot >= 0) {
+                    s1 += to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc);
+                    s2 += to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc);
+                }
                 p1[M * q] = a1;
                 p2[M * q] = a2;
             };
@@ -470,18 +512,24 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
             }
         }
         if constexpr (HEAT) { if (qrow) heat_half(false); }
-        s1 = warp_sum(s1); s2 = warp_sum(s2);
-        if (lane == 0) {
-            double* hst = P.hist + ((size_t)b * (P.nz + 1) + (n + 1)) * 2;
-            atomicAdd(hst + 0, (double)s1 * mb.pscale_step[0]);
-            atomicAdd(hst + 1, (double)s2 * mb.pscale_step[1]);
+        if (slot >= 0) {
+            s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
+            if (lane == 0) {
+                long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+                fix_add(hst + 0, s1);
+                fix_add(hst + 1, s2);
+            }
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
-        table_mul<R, M, PREC, false>(v, hx + m);
+        if constexpr (TS)
+            table_mul_s<R, M, PREC, false>(v, (unsigned)__cvta_generic_to_shared(stab + f * NX + m),
+                                           std::make_integer_sequence<int, R>{});
+        else
+            table_mul<R, M, PREC, false>(v, hx + m);
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
     }
@@ -534,7 +582,6 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
     const MemberDev& mb = P.mem[b];
     const int rot = f ? NX / 2 : 0;
     float2 v[R];
-    float sin0 = 0.f;                                   // ROW_FIRST: sum |A|^2 of the input line
 
     if constexpr (MODE == ROW_FIRST) {
         const float2* src = f ? P.Ain[1] : P.Ain[0];
@@ -545,8 +592,6 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
 #pragma unroll
             for (int q = 0; q < R; ++q) v[q] = make_float2(0.f, 0.f);
         }
-#pragma unroll
-        for (int q = 0; q < R; ++q) sin0 += fmaf(v[q].x, v[q].x, v[q].y * v[q].y);
     } else {
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
 #pragma unroll
@@ -565,7 +610,9 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
     constexpr bool DO_FIRST = (MODE != ROW_FINAL);      // first half of z-step n1
     const int n1 = (MODE == ROW_FIRST) ? 0 : n + 1;
     const float k1h = 0.5f * mb.kap1dz, k2h = 0.5f * mb.kap2dz, g1h = 0.5f * mb.g1dz, g2h = 0.5f * mb.g2dz;
-    float s1 = 0.f, s2 = 0.f;
+    const int slot = DO_SECOND ? rec_slot(P, n + 1) : -1;
+    const float fsc = P.pfix[b];
+    long long s1 = 0, s2 = 0;
     if (P.nzt == 0) {
         // uniform temperature: phi(z) = dk z exactly, all sampled phases are warp-uniform
         PhaseCoef S[3], F[3];
@@ -584,8 +631,10 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
             if (MODE != ROW_FIRST) { a1.y = -a1.y; a2.y = -a2.y; }
             if (DO_SECOND) {
                 rk4_point(a1, a2, S[0], S[1], S[2], g1h, g2h);
-                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
-                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+                if (slot >= 0) {
+                    s1 += to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc);
+                    s2 += to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc);
+                }
             }
             if (DO_FIRST) rk4_point(a1, a2, F[0], F[1], F[2], g1h, g2h);
             p1[M * q] = a1;
@@ -619,8 +668,10 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
                 const float pm = fmaf(0.03125f * dz, fmaf(15.0f, dk0, 9.0f * dkA), ph);
                 const float pb = fmaf(0.5f * dz, dk0 + dkA, ph);
                 half(a1, a2, pa, pm, pb);
-                s1 += fmaf(a1.x, a1.x, a1.y * a1.y);
-                s2 += fmaf(a2.x, a2.x, a2.y * a2.y);
+                if (slot >= 0) {
+                    s1 += to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc);
+                    s2 += to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc);
+                }
                 ph = wrap_2pi(pb);
                 __stcg(phi + M * q, ph);                                     // phi at node n + 1
             }
@@ -635,13 +686,12 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
         }
     }
     // ---- powers at the true nodes (no Parseval factor: the fields are in real space at z_{n+1})
-    {
-        const float t1 = DO_SECOND ? s1 : (f ? 0.f : sin0), t2 = DO_SECOND ? s2 : (f ? sin0 : 0.f);
-        const float w1 = warp_sum(t1), w2 = warp_sum(t2);
+    if (slot >= 0) {
+        s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
         if (lane == 0) {
-            double* hst = P.hist + ((size_t)b * (P.nz + 1) + (DO_SECOND ? n + 1 : 0)) * 2;
-            if (DO_SECOND || G >= 2 || f == 0) atomicAdd(hst + 0, (double)w1 * mb.pscale_in[0]);
-            if (DO_SECOND || G >= 2 || f == 1) atomicAdd(hst + 1, (double)w2 * mb.pscale_in[1]);
+            long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+            fix_add(hst + 0, s1);
+            fix_add(hst + 1, s2);
         }
     }
     if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
@@ -719,9 +769,10 @@ __device__ __forceinline__ void tile_fft(float2 (&v)[FftCfg<N>::R], float2* __re
 // ------------------------------------------------------------------------------------------------
 // NXC: the row length when it is known at compile time (square grids in the persistent kernel: every
 // load / store is then one base register plus an immediate), 0 = take P.nx.
-template <int NY, bool PREC, int NXC>
+template <int NY, bool PREC, int NXC, bool TS = false>
 __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, float2* strip,
-                                         const float4* __restrict__ tws, int trank, int bar_id, int lane) {
+                                         const float4* __restrict__ tws, int trank, int bar_id, int lane,
+                                         const float4* __restrict__ stab = nullptr) {
     using GE = Geo<NY>;
     constexpr int R = GE::R, M = GE::M, SC = GE::SC, CP = GE::CP;
     static_assert(SC == 8 && GE::TW * 4 == M, "tile layout: 8 columns x 4 residues per warp");
@@ -738,9 +789,13 @@ __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, fl
 
 #pragma unroll
     for (int q = 0; q < R; ++q) v[q] = ldcg2(A + q * gstep);
-    table_prefetch<R, M>(h, t);
+    if constexpr (!TS) table_prefetch<R, M>(h, t);
     tile_fft<NY, PREC>(v, colline, tws, t, bar_id);
-    table_mul<R, M, PREC, true>(v, h + t);
+    if constexpr (TS)      // (single simulation: bf is the field; the hy tables follow the two hx tables)
+        table_mul_s<R, M, PREC, true>(v, (unsigned)__cvta_generic_to_shared(stab + (2 + bf) * NY + t),
+                                      std::make_integer_sequence<int, R>{});
+    else
+        table_mul<R, M, PREC, true>(v, h + t);
     tile_fft<NY, PREC>(v, colline, tws, t, bar_id);
     if constexpr (NXC == 0) {
         // runtime stride: recompute the addresses instead of keeping R pointers alive across the transforms
@@ -772,16 +827,17 @@ __device__ __forceinline__ const float4* load_twiddles(unsigned char* smem_raw, 
     return tws;
 }
 
-template <int NX, int MODE, bool PREC, bool HEAT = false>
+template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
 __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float2* smem_cta,
-                                         const float4* __restrict__ tws, int warp, int lane) {
+                                         const float4* __restrict__ tws, int warp, int lane,
+                                         const float4* __restrict__ stab = nullptr) {
     using GE = Geo<NX>;
     int lo, hi;
     cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
     if (slot >= P.row_slots) return;
     for (int it = lo + slot; it < hi; it += P.row_slots)
-        row_item<NX, MODE, PREC, HEAT>(P, it, n, hsel, smem_cta, tws, warp, lane);
+        row_item<NX, MODE, PREC, HEAT, TS>(P, it, n, hsel, smem_cta, tws, warp, lane, stab);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -791,12 +847,12 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
 // (one or two points per thread instead of R/2 per lane of one warp): the RK4 chain, half of a row item's
 // latency, leaves the critical path.  Same per-point arithmetic as row_item<ROW_MID>: bit-identical fields.
 //   phase A  owners: load -> F_x -> line to shared memory          | __syncthreads
-//   phase B  everyone: T / phase / RK4 on the CTA's points, power sums into shared accumulators | __syncthreads
-//   phase C  one thread per (row, field): power to the history;  owners: F_x -> * hx -> store
+//   phase B  everyone: T / phase / RK4 on the CTA's points, power sums (fixed point) to the history | __syncthreads
+//   phase C  owners: F_x -> * hx -> store
 // ------------------------------------------------------------------------------------------------
 template <int NX, bool PREC>
 __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, float2* smem_cta,
-                                              const float4* __restrict__ tws, int warp, int lane, double* s_acc) {
+                                              const float4* __restrict__ tws, int warp, int lane) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG;
     int lo, hi;
@@ -823,7 +879,6 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
 #pragma unroll
         for (int q = 0; q < R; ++q) own[M * q + m] = v[q];     // conj(field), SH rotated by N/2
     }
-    if (threadIdx.x < 2 * GE::ROW_SLOTS * HG) s_acc[threadIdx.x] = 0.0;
     __syncthreads();
 
     // ---- phase B: point idx = ((local item) * HG + row in item) * NX + e; a warp's 32 points share a row
@@ -881,20 +936,22 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
         rk4_point(a1, a2, CA, CM, CB, mb.g1dz, mb.g2dz);
         *q1 = a1;
         *q2 = a2;
-        const float w1 = warp_sum(fmaf(a1.x, a1.x, a1.y * a1.y)), w2 = warp_sum(fmaf(a2.x, a2.x, a2.y * a2.y));
-        if (lane == 0) {
-            atomicAdd(&s_acc[(li * HG + rr) * 2 + 0], (double)w1);
-            atomicAdd(&s_acc[(li * HG + rr) * 2 + 1], (double)w2);
+        // a warp's 32 points share a row, hence a member: one fixed-point atomic per warp and field
+        const int slot = rec_slot(P, n + 1);
+        if (slot >= 0) {
+            const float fsc = P.pfix[b];
+            const long long w1 = warp_sum_ll(to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc));
+            const long long w2 = warp_sum_ll(to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc));
+            if (lane == 0) {
+                long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+                fix_add(hst + 0, w1);
+                fix_add(hst + 1, w2);
+            }
         }
     }
     __syncthreads();
 
     // ---- phase C
-    if ((int)threadIdx.x < nitems * HG * 2) {
-        const int row = lo * HG + (int)threadIdx.x / 2, fld = threadIdx.x & 1;
-        const int b = row / P.ny;
-        atomicAdd(P.hist + ((size_t)b * (P.nz + 1) + (n + 1)) * 2 + fld, s_acc[threadIdx.x] * P.mem[b].pscale_step[fld]);
-    }
     if (has) {
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
@@ -918,9 +975,10 @@ __device__ __forceinline__ void row_pass_paper(const Params& P, int n, float2* s
         row_item_paper<NX, MODE, PREC>(P, it, n, smem_cta, tws, warp, lane);
 }
 
-template <int NY, bool PREC, int NXC>
+template <int NY, bool PREC, int NXC, bool TS = false>
 __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem_cta,
-                                         const float4* __restrict__ tws, int warp, int lane) {
+                                         const float4* __restrict__ tws, int warp, int lane,
+                                         const float4* __restrict__ stab = nullptr) {
     using GE = Geo<NY>;
     int lo, hi;
     cta_range(col_items<NY>(P.batch, P.nx), lo, hi);
@@ -928,7 +986,7 @@ __device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem
     float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
     if (team >= P.col_teams) return;
     for (int it = lo + team; it < hi; it += P.col_teams)
-        col_item<NY, PREC, NXC>(P, it, hsel, strip, tws, trank, 1 + team, lane);
+        col_item<NY, PREC, NXC, TS>(P, it, hsel, strip, tws, trank, 1 + team, lane, stab);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -969,6 +1027,12 @@ __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
     return v;
 }
 
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // Monotonic-counter barrier: instance k is complete when the counter reaches (k+1) * gridDim.x.
 // Arrive = one release reduction (orders the whole CTA's stores, which thread 0 observed through
 // bar.sync, before the increment; no value returned, so no round trip), poll = relaxed loads (one L2 round
@@ -989,18 +1053,24 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
             while (ld_relaxed_u32(P.barrier) < target) {
                 // (the timeout / status checks cost an L2 round trip: not in every poll)
                 if (((++spins) & 31) == 0) {
-                    if (clock64() - t0 > 4000000000LL) { good = 0; atomicExch(P.status, 1); break; }
+                    if (P.spin_limit != 0 && (unsigned long long)(clock64() - t0) > P.spin_limit) {
+                        good = 0; atomicExch(P.status, 1); break;
+                    }
                     if (*((volatile int*)P.status) != 0) { good = 0; break; }
                 }
             }
         }
-        // Acquire side.  Every mutable global array (fields, phi) is read with ld.global.cg (SASS: LDG.STRONG.GPU,
-        // served by L2, never by L1) by threads that pass the bar.sync below only after this poll has
-        // observed the last arrival, whose red.release ordered that CTA's stores before it; the arrays that
-        // L1 may hold (tables, T, member constants) are read-only during a propagate.  A gpu-scope fence here
-        // (MEMBAR + L1 invalidation, ~350 clocks per barrier and cold tables every pass) is therefore only
-        // needed by the letter of the PTX model: SHG_OPT_ACQUIRE_FENCE = 1 turns it on (bit-identical results).
-        if (P.acquire_fence) asm volatile("fence.acq_rel.gpu;" ::: "memory");
+        // Acquire side (SHG_OPT_ACQUIRE_FENCE).  The last arrival's red.release ordered that CTA's stores before
+        // the increment this thread has now observed; the acquire that pairs with it is
+        //   2 (default): one more load of the counter, ld.acquire.gpu -- it reads a value >= target, i.e. from the
+        //      release sequence of every arrival; the bar.sync below carries the ordering to the rest of the CTA
+        //      (causality order is transitive over CTA barriers);
+        //   1: a gpu-scope fence.acq_rel after the relaxed poll (same guarantee, a full MEMBAR);
+        //   0: nothing -- relies on every mutable global array (fields, phi) being read with ld.global.cg
+        //      (SASS LDG.STRONG.GPU: served by L2, never by L1) and on L1 holding only read-only data; outside the
+        //      PTX memory model, kept for measurements (bit-identical results in all three modes).
+        if (P.acquire_fence == 2) (void)ld_acquire_u32(P.barrier);
+        else if (P.acquire_fence == 1) asm volatile("fence.acq_rel.gpu;" ::: "memory");
         ok = good;
         if (P.trace != nullptr && n < P.trace_steps) {
             long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
@@ -1015,19 +1085,34 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
     return ok != 0;
 }
 
-template <int N, bool PREC, bool HEAT = false>
+// TS (single simulation): hx / hy of both fields live in shared memory for the whole run -- 16 B per point and
+// pass that otherwise go through L1 beside the field and temperature streams (ncu, round 1: 35 % L1 hit rate,
+// long_scoreboard on the hx load the top stall of the second row transform).
+template <int N, bool PREC, bool HEAT = false, bool TS = false>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);   // twx == twy on a square grid
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
+    float4* stab = reinterpret_cast<float4*>(smem_raw + Geo<N>::CTA_SMEM);
+    auto stage_tables = [&](int hs) {
+        if constexpr (TS) {
+            for (int i = threadIdx.x; i < 2 * N; i += blockDim.x) {
+                stab[i] = P.hx[hs][i];
+                stab[2 * N + i] = P.hy[hs][i];
+            }
+            __syncthreads();
+        }
+    };
+    stage_tables(P.nz == 1 ? 1 : 0);
     unsigned int epoch = 0;
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        row_pass<N, ROW_MID, PREC, HEAT>(P, n, hsel, smem_cta, tws, warp, lane);
+        if (hsel == 1 && n > 0) stage_tables(1);             // (every warp passed the barrier's closing bar.sync)
+        row_pass<N, ROW_MID, PREC, HEAT, TS>(P, n, hsel, smem_cta, tws, warp, lane, stab);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
+        col_pass<N, PREC, N, TS>(P, hsel, smem_cta, tws, warp, lane, stab);
         if (!grid_barrier(P, epoch, n, 1)) return;
     }
 }
@@ -1036,7 +1121,6 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
 template <int N, bool PREC>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double s_acc[2 * Geo<N>::ROW_SLOTS * Geo<N>::HG];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
@@ -1044,7 +1128,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane, s_acc);
+        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;

@@ -42,18 +42,18 @@ cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-template <bool PREC, bool HEAT>
+template <bool PREC, bool HEAT, bool TS = false>
 cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
-    const int smem = GE::CTA_SMEM;
-    cudaError_t e = set_smem(k_persist<N, PREC, HEAT>, smem);
+    const int smem = TS ? GE::CTA_SMEM_TAB : GE::CTA_SMEM;
+    cudaError_t e = set_smem(k_persist<N, PREC, HEAT, TS>, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persist<N, PREC, HEAT>, GE::THREADS, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persist<N, PREC, HEAT, TS>, GE::THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     Params Pc = P;
     void* args[] = {&Pc};
-    return cudaLaunchCooperativeKernel((const void*)k_persist<N, PREC, HEAT>, dim3(grid), dim3(GE::THREADS), args,
+    return cudaLaunchCooperativeKernel((const void*)k_persist<N, PREC, HEAT, TS>, dim3(grid), dim3(GE::THREADS), args,
                                        (size_t)smem, st);
 }
 }  // namespace
@@ -105,6 +105,7 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
         return cudaLaunchCooperativeKernel(kf, dim3(grid), dim3(GE::THREADS), args, (size_t)smem, st);
     }
     if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
+    if (P.tab_smem && prec) return launch_persist_t<true, false, true>(P, grid, st);
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
 }
 

@@ -17,15 +17,17 @@ struct MemberDev {
     double dk_uniform;         // dk0 + ddk_dT (T_uniform - T_pm), used when nzt == 0
     double dzd;
     float qa1, qb1, qa2, qb2;  // heat source of Eq. 8 per |A_j|^2: q = s1 (qa1 + qb1 s1) + s2 (qa2 + qb2 s2), s_j = |A_j|^2
-    double pscale_in[2];       // (eps0 c n_j/2) dx dy
-    double pscale_step[2];     // exp(-alpha_j dz/2) (eps0 c n_j/2) dx dy  (Parseval: power after the closing half-step)
 };
 
 struct Params {
     int nx, ny, nz, nzt, batch;
     int flat_rows;             // 1: sparse launch, the persistent kernel spreads the nonlinear step over the CTA (row_pass_flat)
     int scheme;                // 0: L/2 - N - L/2 with merged half-steps; 1: the paper's N/2 - L - N/2 (SHG_OPT_SCHEME)
-    int acquire_fence;         // 1: gpu-scope acquire fence after every device-wide barrier (SHG_OPT_ACQUIRE_FENCE)
+    int acquire_fence;         // acquire side of the device-wide barrier (SHG_OPT_ACQUIRE_FENCE): 0 none (L2-only loads),
+                               // 1 gpu-scope fence after the poll, 2 the successful poll is an ld.acquire.gpu
+    int tab_smem;              // 1: the propagator tables hx / hy of member 0 are staged in shared memory (batch == 1)
+    int rec_every, nrec;       // power history: nodes n with n % rec_every == 0, and node nz (slot nrec), are recorded
+    unsigned long long spin_limit;   // device-wide barrier: SM clocks before a timeout is declared (0 = wait forever)
     int row_slots, col_teams;  // slots (warps / warp pairs) and teams per CTA that take items (<= Geo limits)
     float2* A[2];              // working / output fields [batch][ny][nx]
     const float2* Ain[2];      // inputs (Ain[1] may be null)
@@ -37,7 +39,8 @@ struct Params {
     const float4* hx[2];       // [0]=full step dz, [1]=half step: [batch][2][nx]
     const float4* hy[2];       // [batch][2][ny], includes 1/(nx ny)
     const MemberDev* mem;      // [batch]
-    double* hist;              // [batch][nz+1][2]
+    long long* hfix;           // [batch][nrec+1][2] power sums in fixed point: sum over points of rint(|A_j|^2 * pfix[b])
+    const float* pfix;         // [batch] the member's fixed-point scale 2^e (k_input_power), see shg_device.cuh "power sums"
     float* Q;                  // optional heat-source output [batch][nq][ny][nx] (shg_set_heat_output), else null
     const int* qmap;           // [nz]: plane of Q that samples z-step n, or -1
     int nq;

@@ -16,15 +16,18 @@ LIB_PATH = os.path.join(_HERE, "libshg.so")
 
 SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
 OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE, OPT_UNDEPLETED, OPT_SCHEME = 1, 2, 3, 4, 5, 6
+OPT_SPIN_LIMIT, OPT_TABLES_SMEM, OPT_CLUSTER = 7, 8, 9
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
-           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak", "shg_last_launch_count", "shg_destroy", "shg_strerror")
+           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
+           "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
+           "shg_history_nodes")
 
 
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("nzt", C.c_int32),
-                ("batch", C.c_int32)]
+                ("batch", C.c_int32), ("record_every", C.c_int32)]
 
 
 class Crystal(C.Structure):
@@ -63,6 +66,9 @@ def lib():
     L.shg_propagate_host.argtypes = [vp, vp, vp, vp, vp, C.c_int, vp]
     L.shg_power.argtypes = [vp, C.c_int, C.c_double, dp, dp]
     L.shg_power_history.argtypes = [vp, C.c_int, vp]
+    L.shg_synchronize.argtypes = [vp]
+    L.shg_history_length.argtypes = [vp]
+    L.shg_history_nodes.argtypes = [vp, vp]
     L.shg_gaussian_input.argtypes = [vp, vp, C.c_int, vp]
     L.shg_enable_timing.argtypes = [vp, C.c_int]
     L.shg_last_main_loop_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -172,15 +178,24 @@ class Shg:
             raise ValueError("T has %d elements, expected %d" % (numel, want))
 
     # -- shg_propagate: CUDA complex64 tensors [batch][ny][nx]
-    def propagate(self, A1_in, A2_in=None, A1_out=None, A2_out=None, stream=None):
+    def propagate(self, A1_in, A2_in=None, A1_out=None, A2_out=None, stream=None, batch=None):
+        """A1_in None: the library's own Gaussian pump of Eq. 6 (then `batch` members, default the capacity)."""
         import torch
         g = self.grid
-        A1_in = A1_in.reshape(-1, g["ny"], g["nx"])
-        batch = A1_in.shape[0]
-        if A1_out is None:
-            A1_out = torch.empty_like(A1_in)
-        if A2_out is None:
-            A2_out = torch.empty_like(A1_in)
+        if A1_in is None:
+            batch = g["batch"] if batch is None else batch
+            shape = (batch, g["ny"], g["nx"])
+            if A1_out is None:
+                A1_out = torch.empty(shape, dtype=torch.complex64, device="cuda")
+            if A2_out is None:
+                A2_out = torch.empty(shape, dtype=torch.complex64, device="cuda")
+        else:
+            A1_in = A1_in.reshape(-1, g["ny"], g["nx"])
+            batch = A1_in.shape[0]
+            if A1_out is None:
+                A1_out = torch.empty_like(A1_in)
+            if A2_out is None:
+                A2_out = torch.empty_like(A1_in)
         for t in (A1_in, A2_in, A1_out, A2_out):
             if t is not None and t.numel() != batch * g["ny"] * g["nx"]:
                 raise ValueError("field tensors must hold batch*ny*nx complex64 values")
@@ -229,9 +244,20 @@ class Shg:
         return p1.value, p2.value
 
     def power_history(self, member: int = 0) -> np.ndarray:
-        out = np.empty((self.grid["nz"] + 1, 2), dtype=np.float64)
+        out = np.empty((lib().shg_history_length(self._h), 2), dtype=np.float64)
         _check(lib().shg_power_history(self._h, member, C.c_void_p(out.ctypes.data)))
         return out
+
+    def history_nodes(self) -> np.ndarray:
+        """Step indices n of the recorded nodes (shg_grid.record_every)."""
+        out = np.empty(lib().shg_history_length(self._h), dtype=np.int32)
+        _check(lib().shg_history_nodes(self._h, C.c_void_p(out.ctypes.data)))
+        return out
+
+    def synchronize(self):
+        """shg_synchronize: wait for the last propagate; raises if the run failed."""
+        _check(lib().shg_synchronize(self._h))
+        return self
 
     def efficiency(self, member: int = 0) -> float:
         """eta = P2(L) / (P1(0) + P2(0))  (on-grid input power)."""
