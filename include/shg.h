@@ -118,8 +118,9 @@ typedef struct {
                                   one co-resident wave of thread-block clusters, the whole run (opening half-step,
                                   z-loop, closing half-step) is ONE launch of k_cluster: one cluster of 8 or 16
                                   CTAs per member, the fields resident in distributed shared memory, the column
-                                  exchange through DSMEM, cluster barriers instead of device-wide ones; 0: never;
-                                  2: whenever the grid size allows, even if the clusters run in several waves.
+                                  exchange through DSMEM, cluster barriers instead of device-wide ones (nx <= 128);
+                                  0: never; 8 or 16: that cluster size whenever the grid size allows (nx <= 128 for
+                                  8, nx <= 256 for 16), even if the clusters run in several waves.
                                   Same per-point arithmetic as the other kernels: bit-identical fields and powers. */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
@@ -204,6 +205,9 @@ int shg_measure_fp32_peak(double* tflops);
 
 /* Number of kernels the last shg_propagate / shg_propagate_host launched. */
 int shg_last_launch_count(const shg_ctx* ctx);
+
+/* Cluster size (8 or 16) when the last propagate ran in the cluster kernel (SHG_OPT_CLUSTER), else 0. */
+int shg_last_cluster_size(const shg_ctx* ctx);
 
 void shg_destroy(shg_ctx* ctx);
 

@@ -35,6 +35,7 @@ struct Launchers {
     cudaError_t (*row)(const shg::Params&, int, int, int, bool, int, cudaStream_t);
     cudaError_t (*col)(const shg::Params&, int, bool, int, cudaStream_t);
     cudaError_t (*persist)(const shg::Params&, bool, int, cudaStream_t);
+    cudaError_t (*cluster)(const shg::Params&, int, bool, int*, cudaStream_t);
     shg::LaunchInfo (*info)();
 };
 
@@ -42,7 +43,8 @@ bool launchers_for(int n, Launchers* L) {
     switch (n) {
 #define SHG_CASE(N)                                                                                         \
     case N:                                                                                                 \
-        *L = Launchers{shg::launch_row_##N, shg::launch_col_##N, shg::launch_persist_##N, shg::launch_info_##N}; \
+        *L = Launchers{shg::launch_row_##N, shg::launch_col_##N, shg::launch_persist_##N, shg::launch_cluster_##N, \
+                       shg::launch_info_##N};                                                                \
         return true;
         SHG_CASE(64)
         SHG_CASE(128)
@@ -79,7 +81,7 @@ __global__ void k_gaussian(float2* A, const shg::GaussDev* gd, int nx, int ny, i
 // P_j(0) and the member's fixed-point scale (shg_device.cuh, "power sums").  Grid (chunks, batch): every block sums
 // |A_1|^2 and |A_2|^2 over its chunk of the member's input in double, in a fixed order; the last block to finish
 // (ticket counter) adds the chunk sums in chunk order -- deterministic -- and writes
-//   pfix[b] = 2^e with (S_1 + S_2) 2^e in [2^59, 2^60),   hfix[b][0][j] = rint(S_j 2^e).
+//   pfix[b] = 2^e with (S_1 + S_2) 2^e in [2^55, 2^56),   hfix[b][0][j] = rint(S_j 2^e).
 __global__ void __launch_bounds__(256) k_input_power(const float2* __restrict__ A1, const float2* __restrict__ A2,
                                                      size_t np, int nrec, double* part, unsigned int* ticket,
                                                      float* pfix, long long* hfix) {
@@ -120,7 +122,7 @@ __global__ void __launch_bounds__(256) k_input_power(const float2* __restrict__ 
             const double S = S1 + S2;
             int e = 0;
             if (S > 0.0 && S < 1e300) {
-                e = 59 - ilogb(S);
+                e = 55 - ilogb(S);
                 e = e > 120 ? 120 : (e < -120 ? -120 : e);
             }
             pfix[b] = ldexpf(1.0f, e);
@@ -159,7 +161,7 @@ struct shg_ctx {
     bool precise = true;
     int acquire_fence = 2;
     int tables_smem = 1;
-    int cluster_mode = 1;                 // SHG_OPT_CLUSTER: 0 never, 1 auto, 2 whenever the grid size allows
+    int cluster_mode = 1;                 // SHG_OPT_CLUSTER: 0 never, 1 auto, 8 / 16 that cluster size whenever possible
     unsigned long long spin_limit = 4000000000ULL;
     int rec_every = 1, nrec = 0;
     bool undepleted = false;
@@ -204,6 +206,7 @@ struct shg_ctx {
     cudaStream_t last_stream = nullptr;
     int last_batch = 0;
     int last_launches = 0;
+    int last_cluster = 0;               // cluster size of the last propagate (0: batched kernels)
     bool hist_valid = false;
     int last_scheme = 0;
     std::vector<double> hist_host;       // [batch][nrec+1][2], W
@@ -460,7 +463,7 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
             return SHG_OK;
         case SHG_OPT_TABLES_SMEM: ctx->tables_smem = (value != 0); return SHG_OK;
         case SHG_OPT_CLUSTER:
-            if (value < 0 || value > 2) return SHG_EINVAL;
+            if (value != 0 && value != 1 && value != 8 && value != 16) return SHG_EINVAL;
             ctx->cluster_mode = value;
             return SHG_OK;
         case SHG_OPT_SCHEME:
@@ -610,6 +613,45 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         CU(cudaGetLastError());
         ++launches;
     }
+
+    // Small square grids: the whole run of a member in one thread-block cluster (shg_cluster.cuh), one launch.
+    if (ctx->cluster_mode != 0 && ctx->persistent && g.nx == g.ny && g.nx <= 256 && ctx->scheme == 0 && ctx->precise &&
+        !P.Q) {
+        int csize = 0;
+        const int cand[2] = {16, 8};
+        for (int i = 0; i < 2 && csize == 0; ++i) {
+            const int c = cand[i];
+            if (ctx->cluster_mode >= 8 && ctx->cluster_mode != c) continue;
+            int cap = 0;
+            const cudaError_t e = ctx->Lx.cluster(P, c, false, &cap, st);
+            if (e != cudaSuccess) { cudaGetLastError(); continue; }         // this size is not built / not possible
+            // auto: only when every member's cluster is resident at once (a latency optimisation for one or a few
+            // simulations; a sweep of many members fills the device better through the batched kernels), and not
+            // for 256 x 256, where one simulation's arithmetic alone keeps 16 SMs busier than the barriers cost
+            if (ctx->cluster_mode >= 8 ? cap >= 1 : (batch <= cap && g.nx <= 128)) csize = c;
+        }
+        if (csize != 0) {
+            P.trace_grid = batch * csize < ctx->sm_count ? batch * csize : ctx->sm_count;
+            ctx->trace_grid = P.trace_grid;
+            if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
+            const cudaError_t e = ctx->Lx.cluster(P, csize, true, nullptr, st);
+            if (e == cudaSuccess) {
+                ++launches;
+                if (ctx->timing) { CU(cudaEventRecord(ctx->ev[1], st)); ctx->ev_recorded = true; }
+                ctx->last_stream = st;
+                ctx->last_batch = batch;
+                ctx->last_launches = launches;
+                ctx->last_scheme = 0;
+                ctx->last_cluster = csize;
+                ctx->hist_valid = false;
+                return SHG_OK;
+            }
+            if (!coop_unavailable(e) && e != cudaErrorInvalidValue && e != cudaErrorInvalidConfiguration)
+                return cuda_fail(e, "cluster kernel launch");
+            cudaGetLastError();                                             // fall through to the batched kernels
+        }
+    }
+    ctx->last_cluster = 0;
 
     const shg::LaunchInfo ix = ctx->Lx.info(), iy = ctx->Ly.info();
     const int UR = batch * g.ny / ix.rows_per_item;          // row-pass items
@@ -880,5 +922,7 @@ int shg_measure_fp32_peak(double* tflops) {
 }
 
 int shg_last_launch_count(const shg_ctx* ctx) { return ctx ? ctx->last_launches : SHG_EINVAL; }
+
+int shg_last_cluster_size(const shg_ctx* ctx) { return ctx ? ctx->last_cluster : SHG_EINVAL; }
 
 }  // extern "C"

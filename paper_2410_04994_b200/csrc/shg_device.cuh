@@ -216,7 +216,8 @@ __device__ __forceinline__ float warp_sum(float x) {
 // associatively, so the result does not depend on which warp, CTA, launch scheme or kernel summed which points,
 // nor on the arrival order of the atomics: the power history is bit-reproducible and identical between the
 // persistent, per-pass, sparse and cluster kernels.  k_input_power picks e so that the input's total sum maps to
-// [2^59, 2^60): 3 bits of headroom (power does not grow: alpha, beta >= 0) and a resolution of 2^-60 of the input.
+// [2^55, 2^56): 7 bits of headroom (power does not grow, alpha, beta >= 0; a deliberately unstable RK4 step, e.g.
+// nz = 1 at kW powers, may gain a factor ~10) and a resolution of 2^-56 of the input per point.
 __device__ __forceinline__ long long to_fix(float s, float scale) { return __float2ll_rn(s * scale); }
 
 __device__ __forceinline__ long long warp_sum_ll(long long x) {
@@ -515,7 +516,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         if (slot >= 0) {
             s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
             if (lane == 0) {
-                long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+                long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
                 fix_add(hst + 0, s1);
                 fix_add(hst + 1, s2);
             }
@@ -689,7 +690,7 @@ __device__ __forceinline__ void row_item_paper(const Params& P, int item, int n,
     if (slot >= 0) {
         s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
         if (lane == 0) {
-            long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+            long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
             fix_add(hst + 0, s1);
             fix_add(hst + 1, s2);
         }
@@ -943,7 +944,7 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
             const long long w1 = warp_sum_ll(to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc));
             const long long w2 = warp_sum_ll(to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc));
             if (lane == 0) {
-                long long* hst = P.hfix + ((size_t)b * (P.nrec + 1) + slot) * 2;
+                long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
                 fix_add(hst + 0, w1);
                 fix_add(hst + 1, w2);
             }

@@ -5,6 +5,9 @@
 #endif
 
 #include "shg_device.cuh"
+#if SHG_N <= 256
+#include "shg_cluster.cuh"
+#endif
 #include "shg_launch.h"
 
 namespace shg {
@@ -107,6 +110,56 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
     if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
     if (P.tab_smem && prec) return launch_persist_t<true, false, true>(P, grid, st);
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
+}
+
+#if SHG_N <= 256
+namespace {
+// One cluster of C CTAs per member (k_cluster).  max_clusters (if not null) receives how many such clusters the
+// device can hold at once; launch = false only queries.
+template <int C>
+cudaError_t launch_cluster_t(const Params& P, bool launch, int* max_clusters, cudaStream_t st) {
+    using CG = CGeo<N, C>;
+    auto kern = k_cluster<N, C, true>;
+    // at least 120 KB: one CTA per SM, so that the CTAs of a cluster never share an SM's pipes
+    const int smem = CG::SMEM > 120 * 1024 ? CG::SMEM : 120 * 1024;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    if (C > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(P.batch * C));
+    cfg.blockDim = dim3(CG::THREADS);
+    cfg.dynamicSmemBytes = (size_t)smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (max_clusters) {
+        e = cudaOccupancyMaxActiveClusters(max_clusters, kern, &cfg);
+        if (e != cudaSuccess) return e;
+    }
+    if (!launch) return cudaSuccess;
+    return cudaLaunchKernelEx(&cfg, kern, P);
+}
+}  // namespace
+#endif
+
+cudaError_t SHG_CAT(launch_cluster_, SHG_N)(const Params& P, int csize, bool launch, int* max_clusters,
+                                            cudaStream_t st) {
+#if SHG_N <= 128
+    if (csize == 8) return launch_cluster_t<8>(P, launch, max_clusters, st);
+#endif
+#if SHG_N <= 256
+    if (csize == 16) return launch_cluster_t<16>(P, launch, max_clusters, st);
+#endif
+    (void)P; (void)launch; (void)max_clusters; (void)st; (void)csize;
+    return cudaErrorNotSupported;
 }
 
 LaunchInfo SHG_CAT(launch_info_, SHG_N)() {

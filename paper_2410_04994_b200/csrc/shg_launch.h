@@ -22,6 +22,8 @@ struct LaunchInfo {
                                cudaStream_t st);                                                            \
     cudaError_t launch_col_##N(const Params& P, int hsel, bool prec, int grid, cudaStream_t st);           \
     cudaError_t launch_persist_##N(const Params& P, bool prec, int grid, cudaStream_t st);                 \
+    cudaError_t launch_cluster_##N(const Params& P, int csize, bool launch, int* max_clusters,             \
+                                   cudaStream_t st);                                                        \
     LaunchInfo launch_info_##N();
 
 SHG_DECLARE_N(64)

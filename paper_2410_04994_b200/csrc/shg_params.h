@@ -48,6 +48,7 @@ struct Params {
     int* status;               // device status word (barrier timeout)
     long long* trace;          // optional phase timeline of the persistent kernel (SHG_OPT_TRACE), else null:
     int trace_steps;           //   [trace_steps][grid][2 barriers][4] = {clock64 CTA done, clock64 grid done, globaltimer, smid}
+    int trace_grid;            //   CTAs that record (cluster kernel: [trace_steps][trace_grid][8] phase stamps, shg_cluster.cuh)
 };
 
 enum RowMode { ROW_FIRST = 0, ROW_MID = 1, ROW_FINAL = 2 };

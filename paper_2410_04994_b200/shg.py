@@ -22,7 +22,7 @@ EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_tempe
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
            "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
            "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
-           "shg_history_nodes")
+           "shg_history_nodes", "shg_last_cluster_size")
 
 
 class Grid(C.Structure):
@@ -74,6 +74,7 @@ def lib():
     L.shg_last_main_loop_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.shg_read_trace.argtypes = [vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.shg_last_launch_count.argtypes = [vp]
+    L.shg_last_cluster_size.argtypes = [vp]
     L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
     L.shg_measure_fp32_peak.argtypes = [dp]
     L.shg_destroy.argtypes = [vp]
@@ -292,6 +293,9 @@ class Shg:
 
     def last_launch_count(self) -> int:
         return int(lib().shg_last_launch_count(self._h))
+
+    def last_cluster_size(self) -> int:
+        return int(lib().shg_last_cluster_size(self._h))
 
     def close(self):
         if getattr(self, "_h", None):
