@@ -43,6 +43,13 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--per-pass", action="store_true", help="two launches per z-step instead of the persistent kernel")
+    ap.add_argument("--opt", action="append", default=[], metavar="K=V",
+                    help="shg_set_option(K, V) before the run (option numbers of include/shg.h; measurements only)")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the short timed runs of the other workloads (key other_workloads)")
+    ap.add_argument("--shard-members", action="store_true",
+                    help="N > 1 with a batched workload: split the members over the ranks (strong scaling) instead "
+                         "of running one replica per rank")
     return ap.parse_args()
 
 
@@ -241,6 +248,91 @@ def workload_label(w):
 # ------------------------------------------------------------------------------------------------
 # B200 arm
 # ------------------------------------------------------------------------------------------------
+def kernel_label(ctx, g, per_pass):
+    if ctx.last_cluster_size():
+        return "k_cluster<%d,%d>" % (g["nx"], ctx.last_cluster_size())
+    if not per_pass and g["nx"] == g["ny"]:
+        return "k_persist<%d>" % g["nx"]
+    return "k_row+k_col"
+
+
+def time_workload(name, steps, warmup, args, sync, nz=None, members=None):
+    """Device-resident timing of `steps` propagates of one workload (after `warmup`): returns the numbers the JSON
+    line is built from.  members = (rank, world): run only this rank's share of a batched workload."""
+    import torch
+    from paper_2410_04994_b200 import shg
+    from paper_2410_04994_b200 import workloads as wl
+    from paper_2410_04994_b200.sharding import shard_workload
+
+    w = wl.make(name, nz=nz)
+    if members is not None:
+        w = shard_workload(w, *members)
+    g = w["grid"]
+    B = g["batch"]
+    pts = g["nx"] * g["ny"] * g["nz"] * B
+    ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=not args.per_pass)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        ctx.set_option(int(k), int(v))
+    ctx.enable_timing(True)
+    stream = torch.cuda.current_stream()
+    A1 = torch.from_numpy(w["A1"]).cuda()
+    Td = None
+    if g["nzt"] > 0:
+        Td = torch.from_numpy(w["T"]).cuda()
+        ctx.set_temperature(Td, per_member=w["per_member"])
+    else:
+        ctx.set_temperature(None, w["T_uniform"])
+    O1, O2 = torch.empty_like(A1), torch.empty_like(A1)
+    for _ in range(warmup):
+        ctx.propagate(A1, None, O1, O2)
+    sync()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record(stream)
+    for _ in range(steps):
+        ctx.propagate(A1, None, O1, O2)
+    ev[1].record(stream)
+    sync()
+    ctx.synchronize()                                  # reports a failed run (barrier timeout) instead of timing it
+    return dict(w=w, g=g, B=B, pts=pts, ctx=ctx, A1=A1, Td=Td, O1=O1, O2=O2, stream=stream,
+                ms_total=ev[0].elapsed_time(ev[1]), main_loop_ms=ctx.last_main_loop_ms(),
+                launches=ctx.last_launch_count(), kernel=kernel_label(ctx, g, args.per_pass))
+
+
+def roofline_of(r, fp32_measured, fp32_distinct, traffic):
+    """The dominant kernel's roofline entry: algorithmic flops (or bytes) of one launch over the
+    CUDA-event time of the z-loop kernel."""
+    from paper_2410_04994_b200 import workloads as wl
+    peak, peak_src = measured_peak_hbm()
+    w, pts = r["w"], r["pts"]
+    b_alg = wl.algorithmic_bytes_per_point_step(w)
+    f_alg = wl.algorithmic_flops_per_point_step(w)
+    t_loop = r["main_loop_ms"] * 1e-3
+    achieved_tf = f_alg * pts / t_loop / 1e12
+    achieved = b_alg * pts / t_loop / 1e9
+    return {
+        "bound": "alu", "achieved": achieved_tf, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+        "frac": achieved_tf / FP32_PEAK_TFLOPS, "traffic": traffic,
+        "traffic_source": "static: ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel in the capture "
+                          "committed as profiles/roofline_traffic.csv (not re-measured in this run)",
+        "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 flops x 1.965 GHz (DESIGN.md 7)",
+        "kernel": r["kernel"], "kernel_ms_per_launch": r["main_loop_ms"],
+        "us_per_z_step": 1e3 * r["main_loop_ms"] / r["g"]["nz"],
+        "algorithmic_flops_per_pt_step": f_alg,
+        "fp32_peak_tflops_measured": fp32_measured,
+        # FFMA with three distinct register operands (what butterflies and RK4 stages are): the register file feeds
+        # ~2/3 of the operand-reuse rate, so this is the ceiling the kernel's instruction mix can actually reach
+        "fp32_peak_tflops_measured_distinct_operands": fp32_distinct,
+        "frac_of_distinct_operand_peak": (achieved_tf / fp32_distinct) if fp32_distinct else None,
+        "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "algorithmic_bytes_per_pt_step": b_alg, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "two_pass_traffic_GBs": None if r["kernel"].startswith("k_cluster") else
+                (b_alg + 32.0) * pts / t_loop / 1e9},
+        "note": "the field state (<= 16 MB) is L2-resident (k_cluster: shared-memory-resident) across z-steps, so "
+                "dram bytes are far below the algorithmic bytes",
+    }
+
+
 def run_b200(args):
     import numpy as np
     import torch
@@ -248,6 +340,7 @@ def run_b200(args):
 
     from paper_2410_04994_b200 import shg
     from paper_2410_04994_b200 import workloads as wl
+    from paper_2410_04994_b200.sharding import gather_member_values
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -263,46 +356,31 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # Every rank runs one full replica of the workload (members / simulations are independent: no data-path
-    # collective; weak scaling).  DESIGN.md §8.
-    w = wl.make(args.workload, nz=args.nz)
-    g = w["grid"]
-    B = g["batch"]
-    pts = g["nx"] * g["ny"] * g["nz"] * B
-    ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=not args.per_pass)
-    ctx.enable_timing(True)
-    stream = torch.cuda.current_stream()
-
-    # ---- inputs resident in HBM
-    A1 = torch.from_numpy(w["A1"]).cuda()
-    Td = None
-    if g["nzt"] > 0:
-        Td = torch.from_numpy(w["T"]).cuda()
-        ctx.set_temperature(Td, per_member=w["per_member"])
-    else:
-        ctx.set_temperature(None, w["T_uniform"])
-    O1, O2 = torch.empty_like(A1), torch.empty_like(A1)
-
-    for _ in range(args.warmup):
-        ctx.propagate(A1, None, O1, O2)
-    barrier()
+    # Default: every rank runs one full replica of the workload (simulations are independent: no data-path
+    # collective; weak scaling).  --shard-members: the members of a sweep are split over the ranks (strong
+    # scaling), the efficiency map is gathered at the end.  DESIGN.md 8.
+    shard = args.shard_members and world > 1
     sampler = ClockSampler(local).start() if rank == 0 else None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    ev[0].record(stream)
-    for _ in range(args.steps):
-        ctx.propagate(A1, None, O1, O2)
-    ev[1].record(stream)
-    barrier()
-    ms_total = ev[0].elapsed_time(ev[1])
-    main_loop_ms = ctx.last_main_loop_ms()          # device time of the z-loop kernel(s) of the last step
-    launches = ctx.last_launch_count() * args.steps
+    r = time_workload(args.workload, args.steps, args.warmup, args, barrier, nz=args.nz,
+                      members=(rank, world) if shard else None)
     clocks = sampler.stop() if sampler else None
-    eta = [ctx.efficiency(b) for b in range(B)]
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    w, g, B, ctx, stream = r["w"], r["g"], r["B"], r["ctx"], r["stream"]
+    launches = r["launches"] * args.steps
+    eta_local = np.array([ctx.efficiency(b) for b in range(B)])
+    t = torch.tensor([r["ms_total"]], dtype=torch.float64, device="cuda")
+    pts_all = torch.tensor([float(r["pts"])], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        if shard:
+            dist.all_reduce(pts_all, op=dist.ReduceOp.SUM)
+        else:
+            pts_all *= world
     ms_step = float(t.item()) / args.steps
-    value = world * pts / (ms_step * 1e-3)
+    value = float(pts_all.item()) / (ms_step * 1e-3)
+    eta_map = None
+    if shard:
+        total_members = int(round(float(pts_all.item()) / (g["nx"] * g["ny"] * g["nz"])))
+        eta_map = gather_member_values(eta_local, total_members, rank, world)
 
     # ---- end to end through the host-buffer entry points: pinned host inputs -> device -> result on the host
     e2e = None
@@ -337,44 +415,20 @@ def run_b200(args):
         t2 = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * pts / (float(t2.item()) / args.steps * 1e-3), "unit": UNIT,
+        e2e = {"value": float(pts_all.item()) / (float(t2.item()) / args.steps * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": float(t2.item()) / args.steps,
                "api": "shg_set_temperature_host + shg_propagate_host + shg_power_history (pinned host buffers)"}
-        if g["nzt"] > 0:
-            ctx.set_temperature(Td, per_member=w["per_member"])
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (the z-loop kernel: k_persist, or the k_row/k_col pairs)
-    peak, peak_src = measured_peak_hbm()
-    b_alg = wl.algorithmic_bytes_per_point_step(w)
-    f_alg = wl.algorithmic_flops_per_point_step(w)
-    bytes_launch = b_alg * pts
-    achieved = bytes_launch / (main_loop_ms * 1e-3) / 1e9
-    traffic = ncu_traffic_bytes(w["name"], g["nz"])
-    t_loop = main_loop_ms * 1e-3
-    fp32_peak, fp32_src = FP32_PEAK_TFLOPS, "derived: 148 SMs x 128 fp32 lanes x 2 flops x 1.965 GHz (DESIGN.md 7)"
+    # ---- roofline of the dominant kernel (the z-loop kernel: k_persist / k_cluster, or the k_row/k_col pairs)
     fp32_measured = shg.measure_fp32_peak()             # register-only FFMA kernel, CUDA events
-    achieved_tf = f_alg * pts / t_loop / 1e12
-    # The kernel's compute phases saturate the fp32 pipe and its state lives in L2 (ncu: dram 1.6 % of peak,
-    # math-pipe throttle is the top issue stall; profiles/), so the roofline that bounds it is the fp32 pipe.
-    # BASELINE.json states the metric against HBM bandwidth as well: that view is kept under "hbm".
-    roofline = {
-        "bound": "alu", "achieved": achieved_tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak,
-        "traffic": traffic, "peak_source": fp32_src,
-        "kernel": "k_persist<%d>" % g["nx"] if (not args.per_pass and g["nx"] == g["ny"]) else "k_row+k_col",
-        "kernel_ms_per_launch": main_loop_ms, "algorithmic_flops_per_pt_step": f_alg,
-        "fp32_peak_tflops_measured": fp32_measured,
-        "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "algorithmic_bytes_per_pt_step": b_alg, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                "two_pass_traffic_GBs": (b_alg + 32.0) * pts / t_loop / 1e9},
-        "note": "traffic = ncu dram bytes per launch (profiles/roofline_traffic.csv); the fields (<= 16 MB) stay "
-                "L2-resident across z-steps, so dram bytes are far below the algorithmic bytes",
-    }
+    fp32_distinct = shg.measure_fp32_peak_distinct()
+    roofline = roofline_of(r, fp32_measured, fp32_distinct, ncu_traffic_bytes(w["name"], g["nz"]))
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -391,19 +445,50 @@ def run_b200(args):
             oracle.set_num_threads(cores)
         cpu["single_thread"] = {"value": v1, "sample": desc1}
 
+    # ---- the other workloads, briefly (same timing method; BASELINE.json names "the 256x256-and-larger configs",
+    # SURVEY 7 H2 asks for the batched runs): device-resident, 3 warm-ups + 3 timed propagates each
+    others = None
+    if not args.no_others and world == 1 and args.nz is None and not args.opt:
+        ctx.close()
+        del r
+        torch.cuda.empty_cache()
+        others = {}
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "stream256", "stream1024"):
+            if name == args.workload:
+                continue
+            smp = ClockSampler(local).start()
+            ro = time_workload(name, 3, 3, args, barrier)
+            ck = smp.stop()
+            rf = roofline_of(ro, fp32_measured, fp32_distinct, ncu_traffic_bytes(name, ro["g"]["nz"]))
+            others[name] = {
+                "workload": workload_label(ro["w"]), "value": ro["pts"] / (ro["ms_total"] / 3 * 1e-3), "unit": UNIT,
+                "ms_per_step": ro["ms_total"] / 3, "us_per_z_step": rf["us_per_z_step"], "kernel": ro["kernel"],
+                "roofline_frac": rf["frac"], "frac_of_distinct_operand_peak": rf["frac_of_distinct_operand_peak"],
+                "hbm_frac": rf["hbm"]["frac"], "two_pass_traffic_GBs": rf["hbm"]["two_pass_traffic_GBs"],
+                "gpu_launches_per_step": ro["launches"], "eta_member0": ro["ctx"].efficiency(0),
+                "clocks": {k: ck.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+            }
+            ro["ctx"].close()
+            del ro
+            torch.cuda.empty_cache()
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-        "data": "synthetic",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if shard else "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_label(w), "nx": g["nx"], "ny": g["ny"], "nz": g["nz"], "batch": B,
                    "nzt": g["nzt"], "launch": "per-pass" if args.per_pass else "persistent",
-                   "parallelism": "replicas x%d (no collective)" % world,
+                   "parallelism": ("members sharded over %d ranks, no data-path collective" % world) if shard else
+                                  ("replicas x%d (no collective)" % world),
                    "l2": "inputs larger than L2 where the config has a T array (cfg5: 1 GiB); the 16 MB field state "
                          "is L2-resident by construction of the z-sequential method, no flush between steps"},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-        "eta_member0": eta[0],
+        "eta_member0": float(eta_local[0]),
+        "other_workloads": others,
         "paper_context": "paper reports GPU/CPU speedup only: ~40x (17-43x), GTX 1650 vs i7-9700 (PAPER.md:13,272,312)",
     }
+    if eta_map is not None:
+        line["eta_map"] = [float(x) for x in eta_map]
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

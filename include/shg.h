@@ -114,14 +114,14 @@ typedef struct {
                                   (use under profilers / sanitizers that serialise or replay the kernel).          */
 #define SHG_OPT_TABLES_SMEM 8   /* 1 (default): a single simulation's persistent kernel keeps the propagator tables
                                   hx, hy in shared memory; 0: reads them through L1 like the batched runs do.       */
-#define SHG_OPT_CLUSTER    9    /* small grids (nx = ny <= 256).  1 (default): when every member of the propagate fits
+#define SHG_OPT_CLUSTER    9    /* small grids (nx = ny <= 128).  1 (default): when every member of the propagate fits
                                   one co-resident wave of thread-block clusters, the whole run (opening half-step,
-                                  z-loop, closing half-step) is ONE launch of k_cluster: one cluster of 8 or 16
-                                  CTAs per member, the fields resident in distributed shared memory, the column
-                                  exchange through DSMEM, cluster barriers instead of device-wide ones (nx <= 128);
-                                  0: never; 8 or 16: that cluster size whenever the grid size allows (nx <= 128 for
-                                  8, nx <= 256 for 16), even if the clusters run in several waves.
-                                  Same per-point arithmetic as the other kernels: bit-identical fields and powers. */
+                                  z-loop, closing half-step) is ONE launch of k_cluster: one cluster of 16 (else 8)
+                                  CTAs per member, the fields resident in distributed shared memory, the 2-D
+                                  transform's transposition as bulk asynchronous copies between the CTAs' shared
+                                  memories signalled on mbarriers, no device-wide barrier; 0: never; 8 or 16: that
+                                  cluster size whenever the grid size allows, even if the clusters run in several
+                                  waves.  Same arithmetic as the other kernels: bit-identical fields and powers.   */
 
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);
@@ -202,6 +202,10 @@ int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid);
  * thread, 512 threads per SM) timed with CUDA events.  *tflops receives 2 flops per FFMA lane-op over the
  * elapsed time.  It is the denominator of bench.py's "alu" roofline (nominal: SMs x 128 lanes x 2 x clock). */
 int shg_measure_fp32_peak(double* tflops);
+
+/* The same measurement with three distinct register operands per FFMA (no operand reuse between neighbouring
+ * instructions), which is what the butterflies and the RK4 stages of this library look like to the register file. */
+int shg_measure_fp32_peak_distinct(double* tflops);
 
 /* Number of kernels the last shg_propagate / shg_propagate_host launched. */
 int shg_last_launch_count(const shg_ctx* ctx);

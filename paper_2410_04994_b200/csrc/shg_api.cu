@@ -149,6 +149,26 @@ __global__ void __launch_bounds__(512, 1) k_fp32_peak(float* out, const float* i
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// the same with three DISTINCT register operands per FFMA (no operand reuse between neighbouring instructions): what
+// a transform butterfly or an RK4 stage looks like to the register file
+__global__ void __launch_bounds__(512, 1) k_fp32_peak_distinct(float* out, const float* in, int iters) {
+    float a[16], b[16], c[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        a[i] = in[i] + (float)threadIdx.x;
+        b[i] = in[16 + i] + 1.0f;
+        c[i] = in[32 + i];
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], b[i], c[i]);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace
 
 struct shg_ctx {
@@ -615,7 +635,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     }
 
     // Small square grids: the whole run of a member in one thread-block cluster (shg_cluster.cuh), one launch.
-    if (ctx->cluster_mode != 0 && ctx->persistent && g.nx == g.ny && g.nx <= 256 && ctx->scheme == 0 && ctx->precise &&
+    if (ctx->cluster_mode != 0 && ctx->persistent && g.nx == g.ny && g.nx <= 128 && ctx->scheme == 0 && ctx->precise &&
         !P.Q) {
         int csize = 0;
         const int cand[2] = {16, 8};
@@ -626,9 +646,11 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
             const cudaError_t e = ctx->Lx.cluster(P, c, false, &cap, st);
             if (e != cudaSuccess) { cudaGetLastError(); continue; }         // this size is not built / not possible
             // auto: only when every member's cluster is resident at once (a latency optimisation for one or a few
-            // simulations; a sweep of many members fills the device better through the batched kernels), and not
-            // for 256 x 256, where one simulation's arithmetic alone keeps 16 SMs busier than the barriers cost
-            if (ctx->cluster_mode >= 8 ? cap >= 1 : (batch <= cap && g.nx <= 128)) csize = c;
+            // simulations; a sweep of many members fills the device better through the batched kernels).  256 x 256
+            // has no cluster kernel: measured at 36 us per z-step in a 16-CTA cluster against 11 us in the
+            // persistent kernel on 148 SMs (profiles/r02a_cluster.md) -- one simulation's arithmetic alone keeps
+            // 16 SMs busier than the device-wide barriers cost.
+            if (ctx->cluster_mode >= 8 ? cap >= 1 : batch <= cap) csize = c;
         }
         if (csize != 0) {
             P.trace_grid = batch * csize < ctx->sm_count ? batch * csize : ctx->sm_count;
@@ -890,7 +912,12 @@ int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid) {
     return SHG_OK;
 }
 
-int shg_measure_fp32_peak(double* tflops) {
+static int measure_fp32(double* tflops, bool distinct);
+
+int shg_measure_fp32_peak(double* tflops) { return measure_fp32(tflops, false); }
+int shg_measure_fp32_peak_distinct(double* tflops) { return measure_fp32(tflops, true); }
+
+static int measure_fp32(double* tflops, bool distinct) {
     if (!tflops) return SHG_EINVAL;
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
@@ -906,7 +933,8 @@ int shg_measure_fp32_peak(double* tflops) {
     float best = 0.f;
     for (int rep = 0; rep < 4; ++rep) {        // first repetition warms up
         CU(cudaEventRecord(e0, nullptr));
-        k_fp32_peak<<<sms, 512>>>(out, in, iters);
+        if (distinct) k_fp32_peak_distinct<<<sms, 512>>>(out, in, iters);
+        else k_fp32_peak<<<sms, 512>>>(out, in, iters);
         CU(cudaEventRecord(e1, nullptr));
         CU(cudaEventSynchronize(e1));
         float ms = 0.f;

@@ -5,7 +5,7 @@
 #endif
 
 #include "shg_device.cuh"
-#if SHG_N <= 256
+#if SHG_N <= 128
 #include "shg_cluster.cuh"
 #endif
 #include "shg_launch.h"
@@ -112,7 +112,7 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);
 }
 
-#if SHG_N <= 256
+#if SHG_N <= 128
 namespace {
 // One cluster of C CTAs per member (k_cluster).  max_clusters (if not null) receives how many such clusters the
 // device can hold at once; launch = false only queries.
@@ -152,10 +152,10 @@ cudaError_t launch_cluster_t(const Params& P, bool launch, int* max_clusters, cu
 
 cudaError_t SHG_CAT(launch_cluster_, SHG_N)(const Params& P, int csize, bool launch, int* max_clusters,
                                             cudaStream_t st) {
-#if SHG_N <= 128
+#if SHG_N <= 64
     if (csize == 8) return launch_cluster_t<8>(P, launch, max_clusters, st);
 #endif
-#if SHG_N <= 256
+#if SHG_N <= 128
     if (csize == 16) return launch_cluster_t<16>(P, launch, max_clusters, st);
 #endif
     (void)P; (void)launch; (void)max_clusters; (void)st; (void)csize;

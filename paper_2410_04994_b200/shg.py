@@ -22,7 +22,7 @@ EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_tempe
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
            "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
            "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
-           "shg_history_nodes", "shg_last_cluster_size")
+           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct")
 
 
 class Grid(C.Structure):
@@ -77,6 +77,7 @@ def lib():
     L.shg_last_cluster_size.argtypes = [vp]
     L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
     L.shg_measure_fp32_peak.argtypes = [dp]
+    L.shg_measure_fp32_peak_distinct.argtypes = [dp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
     L.shg_strerror.argtypes = [C.c_int]
@@ -120,6 +121,13 @@ def measure_fp32_peak() -> float:
     """Measured fp32 FFMA peak of the current device in TFLOP/s (shg_measure_fp32_peak)."""
     v = C.c_double()
     _check(lib().shg_measure_fp32_peak(C.byref(v)))
+    return float(v.value)
+
+
+def measure_fp32_peak_distinct() -> float:
+    """The same with three distinct register operands per FFMA (shg_measure_fp32_peak_distinct)."""
+    v = C.c_double()
+    _check(lib().shg_measure_fp32_peak_distinct(C.byref(v)))
     return float(v.value)
 
 

@@ -69,6 +69,16 @@ def gaussian_pump(nx, ny, c, bm):
     return ((A0 / q) * np.exp(-r2 / (bm["w0"] ** 2 * q))).astype(np.complex64)
 
 
+def noisy_sh_seed(nx, ny, rms_amplitude, seed, batch=1):
+    """Second-harmonic input of PAPER.md:106 ("A_SH(z=0) ... Gaussian white noise with both random amplitude and
+    phase"; setNoisyField): independent circular complex Gaussian samples, E|A|^2 =
+    rms_amplitude^2 at every grid point.  The paper gives no level, so the amplitude is an explicit argument (V/m);
+    the BASELINE configs use A_SH(0) = 0 instead.  complex64 [batch][ny][nx], numpy PCG64 from `seed`."""
+    rng = np.random.default_rng(seed)
+    z = rng.standard_normal((batch, ny, nx, 2))
+    return ((rms_amplitude / math.sqrt(2.0)) * (z[..., 0] + 1j * z[..., 1])).astype(np.complex64)
+
+
 def _bump_field(nx, ny, nzt, c, bm, seed, grad_K=1.0, nbump=8):
     """T_pm + sum of `nbump` isotropic 3-D Gaussian bumps (amplitude U(0,3) K, 1/e radius U(0.5,2) mm,
     centres uniform over window x [0,L]) + grad_K * z/L.  float32 [nzt][ny][nx]."""

@@ -194,13 +194,21 @@ def test_every_launch_scheme_gives_the_same_bits(name, nz):
     assert cb.last_launch_count() == 4 + 2 * nz and cb.last_cluster_size() == 0
     runs = [("persistent", {shg.OPT_CLUSTER: 0}, 5, 0)]
     n = w["grid"]["nx"]
-    if n <= 128:
+    if n == 64:
         runs += [("auto", {}, 2, 16), ("cluster 8", {shg.OPT_CLUSTER: 8}, 2, 8)]
+    elif n == 128:
+        runs += [("auto", {}, 2, 16), ("cluster 8 asked, not built for 128", {shg.OPT_CLUSTER: 8}, 5, 0)]
     elif n == 256:
-        runs += [("auto", {}, 5, 0), ("cluster 16", {shg.OPT_CLUSTER: 16}, 2, 16)]
+        runs += [("auto", {}, 5, 0), ("cluster 16 asked, not built for 256", {shg.OPT_CLUSTER: 16}, 5, 0)]
     for label, options, launches, csize in runs:
         a1, a2, ah, ca = run_gpu(w, options=options)
         assert ca.last_launch_count() == launches and ca.last_cluster_size() == csize, label
+        if n == 128 and csize:
+            # the 128-point line transform of the cluster kernel sums in a different order (16 lanes x 8 values
+            # instead of 8 x 16): equal to rounding
+            assert rel_l2(a1, b1) < 2e-6 and rel_l2(a2, b2) < 2e-6, label
+            assert np.max(np.abs(ah[0] - bh[0])) < 1e-6 * bh[0][0, 0], label
+            continue
         assert np.array_equal(a1, b1) and np.array_equal(a2, b2), label
         assert np.array_equal(ah[0], bh[0]), label
     # and twice the same run: bit-reproducible history
@@ -208,7 +216,7 @@ def test_every_launch_scheme_gives_the_same_bits(name, nz):
     assert np.array_equal(ah[0], bh[0])
 
 
-@pytest.mark.parametrize("n,cluster", [(64, 1), (64, 0), (64, 8), (128, 1), (128, 0), (128, 8), (256, 0), (256, 16),
+@pytest.mark.parametrize("n,cluster", [(64, 1), (64, 0), (64, 8), (128, 16), (128, 0), (256, 1),
                                        (512, 1), (1024, 1)])
 def test_every_line_length_against_oracle(n, cluster):
     """Short asymmetric run at every supported line length: off-centre beam, SH seed, T array, TPA; the small
@@ -273,14 +281,14 @@ def test_batch_with_per_member_temperature_and_partial_batch():
     A1 = np.stack([wl.gaussian_pump(n, n, c, bm) for bm in beams])
     w = dict(grid=dict(nx=n, ny=n, nz=nz, nzt=nzt, batch=B), crystal=c, beams=beams, T=T, T_uniform=wl.T_PM,
              per_member=True, A1=A1)
-    g1, g2, gh, ctx = run_gpu(w)
-    assert ctx.last_cluster_size() == 16                   # five members: five resident clusters
+    g1, g2, gh, ctx = run_gpu(w, options={shg.OPT_CLUSTER: 16})
+    assert ctx.last_cluster_size() == 16                   # five members: five clusters
     o1, o2, oh = run_oracle(w)
     check(w, g1, g2, gh, o1, o2, oh, tol_field=2e-5, tol_eta=2e-5)
     d1, d2, dh, dctx = run_gpu(w, options={shg.OPT_CLUSTER: 0})       # the batched kernels: same bits
     assert dctx.last_cluster_size() == 0
-    assert np.array_equal(d1, g1) and np.array_equal(d2, g2)
-    assert all(np.array_equal(dh[b], gh[b]) for b in range(B))
+    assert rel_l2(d1, g1) < 2e-6 and rel_l2(d2, g2) < 2e-6          # (128-point lines: equal to rounding, see above)
+    assert all(np.max(np.abs(dh[b] - gh[b])) < 1e-6 * gh[b][0, 0] for b in range(B))
     # propagate only the first 2 members of the capacity-5 context, in place
     A1d = torch.from_numpy(A1[:2].copy()).cuda()
     A2d = torch.zeros_like(A1d)
@@ -396,7 +404,7 @@ def test_barrier_acquire_modes_and_table_placement_are_bit_identical(name, nz):
         assert np.array_equal(a1, b1) and np.array_equal(a2, b2) and np.array_equal(ah[0], bh[0]), options
 
 
-@pytest.mark.parametrize("name,nz,every,cluster", [("cfg2", 23, 5, 1), ("cfg2", 23, 5, 0), ("cfg3", 12, 4, 0),
+@pytest.mark.parametrize("name,nz,every,cluster", [("cfg2", 23, 5, 16), ("cfg2", 23, 5, 0), ("cfg3", 12, 4, 0),
                                                    ("cfg1", 9, 100, 1), ("cfg5", 7, 3, 0)])
 def test_record_every_thins_the_history_without_changing_it(name, nz, every, cluster):
     """shg_grid.record_every: nodes 0, r, 2r, .. and nz are recorded; they carry the same numbers as the full
@@ -522,6 +530,23 @@ def test_stream_workloads_reduced_batch_against_oracle(name):
     g1, g2, gh, _ = run_gpu(w)
     o1, o2, oh = run_oracle(w)
     check(w, g1, g2, gh, o1, o2, oh, tol_field=2e-5, tol_eta=2e-5)
+
+
+def test_noisy_second_harmonic_seed_matches_oracle():
+    """P:106 / P:380-385 (setNoisyField): the SH input is complex Gaussian white noise.  cfg2 with a seeded noise
+    seed at 1e-3 of the pump's peak amplitude: white noise fills the whole spectrum up to Nyquist, the hardest
+    input for the transforms and the propagator tables."""
+    w = wl.make("cfg2", nz=200)
+    peak = float(np.max(np.abs(w["A1"])))
+    A2 = wl.noisy_sh_seed(128, 128, 1e-3 * peak, seed=106)
+    assert abs(np.sqrt(np.mean(np.abs(A2) ** 2)) / (1e-3 * peak) - 1) < 0.02 and abs(np.mean(A2)) < 0.05 * 1e-3 * peak
+    for cluster in (16, 0):
+        g1, g2, gh, _ = run_gpu(w, A2=A2, options={shg.OPT_CLUSTER: cluster})
+        if cluster == 16:
+            o1, o2, oh = run_oracle(w, A2=A2)
+            z1, z2, _ = run_oracle(w)
+            assert rel_l2(o2, z2) > 1e-3                                  # the seed matters
+        check(w, g1, g2, gh, o1, o2, oh)
 
 
 def test_undepleted_pump_option_matches_oracle_switch():
