@@ -10,6 +10,7 @@
 #include <string>
 #include <vector>
 
+#include "shg_device.cuh"   // uniform_coefs (k_uniform_coefs); no kernel template is instantiated here
 #include "shg_launch.h"
 #include "shg_params.h"
 
@@ -133,6 +134,18 @@ __global__ void __launch_bounds__(256) k_input_power(const float2* __restrict__ 
     }
 }
 
+// nzt == 0: coupling coefficients of every (member, z-step), see shg_device.cuh: uniform_coefs
+__global__ void k_uniform_coefs(const shg::MemberDev* mem, float4* ucoef, int nz, int batch) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nz * batch) return;
+    const int b = i / nz, n = i - b * nz;
+    shg::PhaseCoef a, c, d;
+    shg::uniform_coefs(mem[b], n, a, c, d);
+    ucoef[(size_t)i * 3 + 0] = make_float4(a.u1x, a.u1y, a.u2x, a.u2y);
+    ucoef[(size_t)i * 3 + 1] = make_float4(c.u1x, c.u1y, c.u2x, c.u2y);
+    ucoef[(size_t)i * 3 + 2] = make_float4(d.u1x, d.u1y, d.u2x, d.u2y);
+}
+
 // fp32 pipe peak: 16 independent FFMA chains per thread, nothing else in the loop
 __global__ void __launch_bounds__(512, 1) k_fp32_peak(float* out, const float* in, int iters) {
     float a[16];
@@ -197,6 +210,7 @@ struct shg_ctx {
     float4* d_hy[2] = {nullptr, nullptr};
     shg::MemberDev* d_mem = nullptr;
     shg::GaussDev* d_gauss = nullptr;
+    float4* d_ucoef = nullptr;           // nzt == 0: [batch][nz][3] coupling coefficients per z-step
     float* d_phi = nullptr;
     long long* d_hfix = nullptr;         // [batch][nrec+1][2] fixed-point power sums
     float* d_pfix = nullptr;             // [batch] fixed-point scale 2^e of each member
@@ -345,6 +359,12 @@ int upload_tables(shg_ctx* ctx) {
     }
     CU(cudaMemcpy(ctx->d_mem, mem.data(), sizeof(shg::MemberDev) * B, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_gauss, gs.data(), sizeof(shg::GaussDev) * B, cudaMemcpyHostToDevice));
+    if (ctx->d_ucoef) {
+        const int total = g.nz * B;
+        k_uniform_coefs<<<(total + 127) / 128, 128>>>(ctx->d_mem, ctx->d_ucoef, g.nz, B);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(nullptr));
+    }
     ctx->tables_dirty = false;
     return SHG_OK;
 }
@@ -360,6 +380,7 @@ void free_ctx(shg_ctx* ctx) {
     }
     cudaFree(ctx->d_mem);
     cudaFree(ctx->d_gauss);
+    cudaFree(ctx->d_ucoef);
     cudaFree(ctx->d_phi);
     cudaFree(ctx->d_hfix);
     cudaFree(ctx->d_pfix);
@@ -450,6 +471,7 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     alloc((void**)&ctx->d_mem, sizeof(shg::MemberDev) * B);
     alloc((void**)&ctx->d_gauss, sizeof(shg::GaussDev) * B);
     if (grid->nzt > 0) alloc((void**)&ctx->d_phi, sizeof(float) * (size_t)B * np);
+    else alloc((void**)&ctx->d_ucoef, sizeof(float4) * (size_t)B * grid->nz * 3);
     alloc((void**)&ctx->d_hfix, sizeof(long long) * (size_t)B * (ctx->nrec + 1) * 2);
     alloc((void**)&ctx->d_pfix, sizeof(float) * B);
     alloc((void**)&ctx->d_inpart, sizeof(double) * (size_t)B * 64 * 2);
@@ -609,6 +631,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     P.twx = ctx->d_twx; P.twy = ctx->d_twy;
     for (int hs = 0; hs < 2; ++hs) { P.hx[hs] = ctx->d_hx[hs]; P.hy[hs] = ctx->d_hy[hs]; }
     P.mem = ctx->d_mem;
+    P.ucoef = ctx->d_ucoef;
     P.hfix = ctx->d_hfix; P.pfix = ctx->d_pfix;
     P.rec_every = ctx->rec_every; P.nrec = ctx->nrec;
     P.spin_limit = ctx->spin_limit;

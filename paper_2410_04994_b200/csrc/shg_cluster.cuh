@@ -211,15 +211,19 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
     stage_tables(1);
     cluster_sync_all();                                              // every CTA's mbarriers exist before any copy is sent
 
-    // Send the C blocks of a staging buffer: block d goes to slot `rank` of CTA d's receive buffer.  Called by the
-    // owner warps after they wrote the staging buffer (generic proxy -> async proxy fence, owners' barrier).
+    // Send the C blocks of a staging buffer: block d goes to slot `rank` of CTA d's receive buffer.  Called by ALL
+    // warps once the owner warps have written the staging buffer (their generic-proxy writes fenced towards the async
+    // proxy).  A warp issues its bulk copies one lane after the other (~60 clocks each: 16 copies from one warp
+    // cost ~1000 clocks, tests/probes/dsmem_alltoall.cu), so the C copies are spread over all warps of the CTA.
     auto send_blocks = [&](float2* xbuf, float2* recv, unsigned bar) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        named_barrier(1, FW * 32);
-        if (warp == 0 && lane < C) {
-            const unsigned src = (unsigned)__cvta_generic_to_shared(xbuf + lane * BLK);
-            const unsigned dst = map_to_rank((unsigned)__cvta_generic_to_shared(recv + rank * BLK), (unsigned)lane);
-            bulk_copy_to_rank(dst, src, BLK_BYTES, map_to_rank(bar, (unsigned)lane));
+        if (owner) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        constexpr int PER_WARP = (C + WARPS - 1) / WARPS;
+        const int d = warp * PER_WARP + lane;
+        if (lane < PER_WARP && d < C) {
+            const unsigned src = (unsigned)__cvta_generic_to_shared(xbuf + d * BLK);
+            const unsigned dst = map_to_rank((unsigned)__cvta_generic_to_shared(recv + rank * BLK), (unsigned)d);
+            bulk_copy_to_rank(dst, src, BLK_BYTES, map_to_rank(bar, (unsigned)d));
         }
     };
     // wait for the blocks of all C senders, then (thread 0) arm the barrier for its next phase
@@ -270,8 +274,8 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
                 const int y = F::eout(q, m);
                 xcol[(((y / NR) * 2 + cf) * NR + y % NR) * NR + ccl] = v[q];
             }
-            send_blocks(xcol, rowbuf, bar_row);
         }
+        send_blocks(xcol, rowbuf, bar_row);
     };
     // the CTA's row (rf, rr) from the blocks of the column owners: element kx = M q + m
     auto load_row = [&](float2 (&v)[R]) {
@@ -327,23 +331,12 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
     };
     // What z-step n needs besides its fields, computed while the blocks of the previous pass are in flight.
     // Uniform temperature: phi(z) = dk z exactly, the same three phases at every point -- ONE lane (of a warp that
-    // holds no lines) evaluates them in double and leaves the twelve coefficients in shared memory.
+    // holds no lines) fetches the step's twelve coefficients from the table and leaves them in shared memory.
     auto prepare_step = [&](int n) {
         if (P.nzt == 0) {
             if (tid == THREADS - 32) {
-                const double TWO_PI = 6.283185307179586476925286766559;
-                double pa = mb.dk_uniform * ((double)n * mb.dzd);
-                double pm = mb.dk_uniform * (((double)n + 0.5) * mb.dzd);
-                double pb = mb.dk_uniform * (((double)n + 1.0) * mb.dzd);
-                pa -= TWO_PI * rint(pa / TWO_PI);
-                pm -= TWO_PI * rint(pm / TWO_PI);
-                pb -= TWO_PI * rint(pb / TWO_PI);
-                float ca, sa, cm, sm, cb, sb;
-                sincosf((float)pa, &sa, &ca);
-                sincosf((float)pm, &sm, &cm);
-                sincosf((float)pb, &sb, &cb);
-                const PhaseCoef a = phase_coef(ca, sa, k1dz, k2dz), c = phase_coef(cm, sm, k1dz, k2dz),
-                                d = phase_coef(cb, sb, k1dz, k2dz);
+                PhaseCoef a, c, d;
+                load_uniform_coefs(P, b, n, a, c, d);
                 s_coef[0] = a.u1x; s_coef[1] = a.u1y; s_coef[2] = a.u2x; s_coef[3] = a.u2y;
                 s_coef[4] = c.u1x; s_coef[5] = c.u1y; s_coef[6] = c.u2x; s_coef[7] = c.u2y;
                 s_coef[8] = d.u1x; s_coef[9] = d.u1y; s_coef[10] = d.u2x; s_coef[11] = d.u2y;
@@ -370,8 +363,8 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
         table_mul_s<R, 8, PREC, false>(v, (unsigned)__cvta_generic_to_shared(stab + rf * N + F::tab_lane(m)),
                                        std::make_integer_sequence<int, R>{});
         stage_row_result(v);
-        send_blocks(xrow, colbuf, bar_col);
     }
+    send_blocks(xrow, colbuf, bar_col);
     if (P.nzt != 0) {                                                // dk at node 0, raw T of node 1
         load_T(0);
 #pragma unroll
@@ -452,11 +445,10 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
             table_mul_s<R, 8, PREC, false>(v, (unsigned)__cvta_generic_to_shared(stab + rf * N + F::tab_lane(m)),
                                            std::make_integer_sequence<int, R>{});
             stage_row_result(v);
-            send_blocks(xrow, colbuf, bar_col);
         }
+        send_blocks(xrow, colbuf, bar_col);
         stamp(3);
         if (P.nzt != 0 && n + 2 <= P.nz) load_T(n + 2);              // raw T for dk(z_{n+2}), used after the column pass
-        if (owner) { /* (the wait for the column blocks is inside column_pass) */ }
         column_pass();
         stamp(5);
         if (n + 1 < P.nz) prepare_step(n + 1);
