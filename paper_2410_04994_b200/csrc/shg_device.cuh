@@ -374,7 +374,8 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
 template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
 __device__ __forceinline__ void row_item(const Params& P, int item, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
-                                         const float4* __restrict__ stab = nullptr) {
+                                         const float4* __restrict__ stab = nullptr,
+                                         unsigned long long* s_pow = nullptr) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
     const int g = lane / M, m = lane % M;
@@ -535,9 +536,16 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         if (slot >= 0) {
             s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
             if (lane == 0) {
-                long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
-                fix_add(hst + 0, s1);
-                fix_add(hst + 1, s2);
+                if (s_pow) {
+                    // single simulation: the CTA's sums meet in shared memory; one global atomic per CTA, field
+                    // and step (flush_powers) instead of one per warp on the same two history words
+                    atomicAdd(s_pow + 0, (unsigned long long)s1);
+                    atomicAdd(s_pow + 1, (unsigned long long)s2);
+                } else {
+                    long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
+                    fix_add(hst + 0, s1);
+                    fix_add(hst + 1, s2);
+                }
             }
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
@@ -850,14 +858,25 @@ __device__ __forceinline__ const float4* load_twiddles(unsigned char* smem_raw, 
 template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
 __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
-                                         const float4* __restrict__ stab = nullptr) {
+                                         const float4* __restrict__ stab = nullptr,
+                                         unsigned long long* s_pow = nullptr) {
     using GE = Geo<NX>;
     int lo, hi;
     cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
     if (slot >= P.row_slots) return;
     for (int it = lo + slot; it < hi; it += P.row_slots)
-        row_item<NX, MODE, PREC, HEAT, TS>(P, it, n, hsel, smem_cta, tws, warp, lane, stab);
+        row_item<NX, MODE, PREC, HEAT, TS>(P, it, n, hsel, smem_cta, tws, warp, lane, stab, s_pow);
+}
+
+// single simulation (batch == 1): the CTA's shared power sums of node n + 1 go to the history (after a CTA barrier)
+__device__ __forceinline__ void flush_powers(const Params& P, int n, unsigned long long* s_pow) {
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        const int slot = rec_slot(P, n + 1);
+        if (slot >= 0) fix_add(P.hfix + (long long)slot * 2 + threadIdx.x, (long long)s_pow[threadIdx.x]);
+        s_pow[threadIdx.x] = 0ull;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -872,7 +891,8 @@ __device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float
 // ------------------------------------------------------------------------------------------------
 template <int NX, bool PREC>
 __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, float2* smem_cta,
-                                              const float4* __restrict__ tws, int warp, int lane) {
+                                              const float4* __restrict__ tws, int warp, int lane,
+                                              unsigned long long* s_acc) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG;
     int lo, hi;
@@ -887,6 +907,8 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
     float2 v[R];
     float2* A = nullptr;
     const float4* hx = nullptr;
+    // (read last in phase C of the previous step, two device-wide barriers ago)
+    if (threadIdx.x < 2 * GE::ROW_SLOTS * HG) s_acc[threadIdx.x] = 0ull;
     if (has) {
         const int item = lo + slot;
         const int b = (item * HG) / P.ny;
@@ -949,22 +971,29 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
         rk4_point(a1, a2, CA, CM, CB, mb.g1dz, mb.g2dz);
         *q1 = a1;
         *q2 = a2;
-        // a warp's 32 points share a row, hence a member: one fixed-point atomic per warp and field
-        const int slot = rec_slot(P, n + 1);
-        if (slot >= 0) {
+        // a warp's 32 points share a row: fixed-point warp sums into the row's shared accumulators
+        if (rec_slot(P, n + 1) >= 0) {
             const float fsc = P.pfix[b];
             const long long w1 = warp_sum_ll(to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc));
             const long long w2 = warp_sum_ll(to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc));
             if (lane == 0) {
-                long long* hst = P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2;
-                fix_add(hst + 0, w1);
-                fix_add(hst + 1, w2);
+                atomicAdd(&s_acc[(li * HG + rr) * 2 + 0], (unsigned long long)w1);
+                atomicAdd(&s_acc[(li * HG + rr) * 2 + 1], (unsigned long long)w2);
             }
         }
     }
     __syncthreads();
 
-    // ---- phase C
+    // ---- phase C: one thread per (row, field) adds the row's sum to the history (2 global atomics per row instead
+    // of 2 per warp: they all hit the member's two history words, and the barrier's release waits for them)
+    if ((int)threadIdx.x < nitems * HG * 2) {
+        const int slot = rec_slot(P, n + 1);
+        if (slot >= 0) {
+            const int row = lo * HG + (int)threadIdx.x / 2, fld = threadIdx.x & 1;
+            const int b = row / P.ny;
+            fix_add(P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2 + fld, (long long)s_acc[threadIdx.x]);
+        }
+    }
     if (has) {
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
@@ -1009,8 +1038,12 @@ template <int NX, int MODE, bool PREC, bool HEAT = false>
 __global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row(Params P, int n, int hsel) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ unsigned long long s_pow[2];
+    if (threadIdx.x < 2) s_pow[threadIdx.x] = 0ull;
     const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
-    row_pass<NX, MODE, PREC, HEAT>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
+    unsigned long long* sp = (MODE == ROW_MID && P.batch == 1) ? s_pow : nullptr;
+    row_pass<NX, MODE, PREC, HEAT>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane, nullptr, sp);
+    if (sp) flush_powers(P, n, sp);
 }
 
 template <int NX, int MODE, bool PREC>
@@ -1117,13 +1150,18 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
             __syncthreads();
         }
     };
+    __shared__ unsigned long long s_pow[2];
+    if (threadIdx.x < 2) s_pow[threadIdx.x] = 0ull;
+    unsigned long long* sp = (P.batch == 1) ? s_pow : nullptr;
+    __syncthreads();
     stage_tables(P.nz == 1 ? 1 : 0);
     unsigned int epoch = 0;
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         if (hsel == 1 && n > 0) stage_tables(1);             // (every warp passed the barrier's closing bar.sync)
-        row_pass<N, ROW_MID, PREC, HEAT, TS>(P, n, hsel, smem_cta, tws, warp, lane, stab);
+        row_pass<N, ROW_MID, PREC, HEAT, TS>(P, n, hsel, smem_cta, tws, warp, lane, stab, sp);
+        if (sp) flush_powers(P, n, sp);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N, TS>(P, hsel, smem_cta, tws, warp, lane, stab);
         if (!grid_barrier(P, epoch, n, 1)) return;
@@ -1134,6 +1172,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
 template <int N, bool PREC>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ unsigned long long s_acc[2 * Geo<N>::ROW_SLOTS * Geo<N>::HG];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
@@ -1141,7 +1180,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane);
+        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane, s_acc);
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;
