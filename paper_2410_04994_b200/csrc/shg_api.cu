@@ -624,6 +624,8 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const shg_grid& g = ctx->g;
     shg::Params P{};
     P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.nzt = g.nzt; P.batch = batch;
+    P.ny_log2 = 0;
+    while ((1 << P.ny_log2) < g.ny) ++P.ny_log2;
     P.A[0] = (float2*)A1_out; P.A[1] = (float2*)A2_out;
     P.Ain[0] = (const float2*)A1_in; P.Ain[1] = (const float2*)A2_in;
     P.T = ctx->d_T; P.T_per_member = ctx->T_per_member;

@@ -32,6 +32,15 @@
 
 namespace shg {
 
+// Build-time diagnostic (SHG_NVCC_EXTRA=-DSHG_WTRACE, not in the product build): lane 0 of every warp stamps the SM
+// clock at eight points of a row item of z-steps 100..163 into the tail of the SHG_OPT_TRACE buffer (run with
+// SHG_OPT_TRACE = 4096 and nz >= 4100; layout [64][grid][16 warps][8] after the first 200 x grid x 8 words).
+#ifdef SHG_WTRACE
+#define SHG_WT(i) do { if (wt && lane == 0) wt[i] = clock64(); } while (0)
+#else
+#define SHG_WT(i) do { } while (0)
+#endif
+
 template <int N> struct FftCfg;
 template <> struct FftCfg<64>   { static constexpr int R = 8,  M = 8;  };
 template <> struct FftCfg<128>  { static constexpr int R = 16, M = 8;  };
@@ -361,6 +370,33 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
     return t;
 }
 
+// Scalars that are the same for every item of a CTA's pass.  Computing them per item costs two 64-bit and one
+// 32-bit integer division (~400 instructions) at the head of every row item, where all warps of the CTA execute them
+// at the same time right after a device-wide barrier and nothing else can be issued (measured on cfg5 with per-warp
+// clock stamps: ~2.5 K of the row pass's 39.5 K clocks).  They live in shared memory instead: the ranges are fixed
+// for the run, the step's entries are written by ONE thread while it waits at the barrier before the pass.
+struct StepCtx {
+    int row_lo, row_hi, col_lo, col_hi;    // cta_range of the row items / column strips
+    TNode ta, tb;                          // temperature planes of step nodes n and n + 1 (G15)
+    int slot;                              // rec_slot(n + 1): history slot of P_j(z_{n+1}), -1 = not recorded
+};
+
+__device__ __forceinline__ void cta_range(int U, int& lo, int& hi);
+template <int NX> __host__ __device__ inline int row_items(int batch, int ny);
+template <int NY> __host__ __device__ inline int col_items(int batch, int nx);
+
+template <int NX> __device__ __forceinline__ void ctx_rows(const Params& P, StepCtx& sc) {
+    cta_range(row_items<NX>(P.batch, P.ny), sc.row_lo, sc.row_hi);
+}
+template <int NY> __device__ __forceinline__ void ctx_cols(const Params& P, StepCtx& sc) {
+    cta_range(col_items<NY>(P.batch, P.nx), sc.col_lo, sc.col_hi);
+}
+__device__ __forceinline__ void ctx_step(const Params& P, StepCtx& sc, int n) {
+    sc.ta = t_node(n, P.nz, P.nzt);
+    sc.tb = t_node(n + 1, P.nz, P.nzt);
+    sc.slot = rec_slot(P, n + 1);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Row pass, one item = HG rows x both fields.  Lane group g of the warp holds one line: field f, row r.
 // (G == 1: the item is one row and the two warps of a pair hold its two fields.)
@@ -372,7 +408,7 @@ __device__ __forceinline__ TNode t_node(int n, int nz, int nzt) {
 // HEAT: also write the heat source of Eq. 8 (a separate instantiation: the common path carries none of it).
 // TS: the hx tables are read from shared memory (stab: [2][NX] float4, single simulation) instead of global / L1.
 template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
-__device__ __forceinline__ void row_item(const Params& P, int item, int n, int hsel, float2* smem_cta,
+__device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int item, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
                                          const float4* __restrict__ stab = nullptr,
                                          unsigned long long* s_pow = nullptr) {
@@ -382,8 +418,8 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
     const int f = (G >= 2) ? g / HG : (warp & 1);
     const int r = (G >= 2) ? g % HG : 0;
     const int row = item * HG + r;                            // over [batch * ny]
-    const int b = (item * HG) / P.ny;
-    const int y = row - b * P.ny;
+    const int b = (item * HG) >> P.ny_log2;                   // (ny is a power of two)
+    const int y = row - (b << P.ny_log2);
     const size_t rbase = (size_t)row * NX;
     float2* own = smem_cta + (size_t)warp * (G * NP) + g * NP;
     float2* par = (G >= 2) ? smem_cta + (size_t)warp * (G * NP) + (g ^ HG) * NP
@@ -421,6 +457,10 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
     }
 
     if constexpr (MODE == ROW_MID) {
+#ifdef SHG_WTRACE
+        long long* wt = (P.trace && n >= 100 && n < 164) ? P.trace + 200 * (size_t)gridDim.x * 8 + (((size_t)(n - 100) * gridDim.x + blockIdx.x) * 16 + warp) * 8 : nullptr;
+#endif
+        SHG_WT(0);
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
         const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
@@ -431,7 +471,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
         // registers allow), those of the second right after it; inside the loop two points ahead
         const size_t plane = (size_t)P.ny * NX;
         const size_t pbase = (size_t)y * NX + rot + m;
-        const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
+        const TNode ta = sc.ta, tb = sc.tb;
         const float* Ta = nullptr;
         const float* Tn = nullptr;
         float* phi = nullptr;
@@ -443,7 +483,9 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
             phi = P.phi + (size_t)b * plane + pbase;
             if constexpr (R < 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
         }
+        SHG_WT(1);
         warp_fft<NX, PREC>(v, own, tws, m);
+        SHG_WT(2);
         if (P.nzt != 0) {
             // (a 32-value line leaves no registers to carry operands across the transform)
             if constexpr (R >= 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
@@ -453,13 +495,14 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
 #pragma unroll
         for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
+        SHG_WT(3);
 
         // ---- nonlinear step on elements e = M q + m + f N/2, q < R/2: own lower half, partner's upper half.
         // p1 / p2 address A1 / A2 of this lane's points whichever side it is on (no value selects).
         float2* p1 = (f ? par + M * H : own) + m;
         float2* p2 = (f ? own : par + M * H) + m;
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz, g1 = mb.g1dz, g2 = mb.g2dz;
-        const int slot = rec_slot(P, n + 1);                  // warp-uniform: is P_j(z_{n+1}) recorded?
+        const int slot = sc.slot;                             // warp-uniform: is P_j(z_{n+1}) recorded?
         const float fsc = P.pfix[b];
         long long s1 = 0, s2 = 0;
         // Heat source of Eq. 8 for the plane that samples this z-step, if any (warp-uniform): half of
@@ -533,6 +576,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
             }
         }
         if constexpr (HEAT) { if (qrow) heat_half(false); }
+        SHG_WT(4);
         if (slot >= 0) {
             s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
             if (lane == 0) {
@@ -549,10 +593,12 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
             }
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
+        SHG_WT(5);
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
+        SHG_WT(6);
         if constexpr (TS)
             table_mul_s<R, M, PREC, false>(v, (unsigned)__cvta_generic_to_shared(stab + f * NX + m),
                                            std::make_integer_sequence<int, R>{});
@@ -560,6 +606,7 @@ __device__ __forceinline__ void row_item(const Params& P, int item, int n, int h
             table_mul<R, M, PREC, false>(v, hx + m);
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
+        SHG_WT(7);
     }
 }
 
@@ -856,24 +903,23 @@ __device__ __forceinline__ const float4* load_twiddles(unsigned char* smem_raw, 
 }
 
 template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
-__device__ __forceinline__ void row_pass(const Params& P, int n, int hsel, float2* smem_cta,
+__device__ __forceinline__ void row_pass(const Params& P, const StepCtx& sc, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
                                          const float4* __restrict__ stab = nullptr,
                                          unsigned long long* s_pow = nullptr) {
     using GE = Geo<NX>;
-    int lo, hi;
-    cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
+    const int lo = sc.row_lo, hi = sc.row_hi;
     const int slot = (GE::G >= 2) ? warp : (warp >> 1);
     if (slot >= P.row_slots) return;
     for (int it = lo + slot; it < hi; it += P.row_slots)
-        row_item<NX, MODE, PREC, HEAT, TS>(P, it, n, hsel, smem_cta, tws, warp, lane, stab, s_pow);
+        row_item<NX, MODE, PREC, HEAT, TS>(P, sc, it, n, hsel, smem_cta, tws, warp, lane, stab, s_pow);
 }
 
 // single simulation (batch == 1): the CTA's shared power sums of node n + 1 go to the history (after a CTA barrier)
-__device__ __forceinline__ void flush_powers(const Params& P, int n, unsigned long long* s_pow) {
+__device__ __forceinline__ void flush_powers(const Params& P, const StepCtx& sc, unsigned long long* s_pow) {
     __syncthreads();
     if (threadIdx.x < 2) {
-        const int slot = rec_slot(P, n + 1);
+        const int slot = sc.slot;
         if (slot >= 0) fix_add(P.hfix + (long long)slot * 2 + threadIdx.x, (long long)s_pow[threadIdx.x]);
         s_pow[threadIdx.x] = 0ull;
     }
@@ -890,13 +936,12 @@ __device__ __forceinline__ void flush_powers(const Params& P, int n, unsigned lo
 //   phase C  owners: F_x -> * hx -> store
 // ------------------------------------------------------------------------------------------------
 template <int NX, bool PREC>
-__device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, float2* smem_cta,
+__device__ __forceinline__ void row_pass_flat(const Params& P, const StepCtx& sc, int n, int hsel, float2* smem_cta,
                                               const float4* __restrict__ tws, int warp, int lane,
                                               unsigned long long* s_acc) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG;
-    int lo, hi;
-    cta_range(row_items<NX>(P.batch, P.ny), lo, hi);
+    const int lo = sc.row_lo, hi = sc.row_hi;
     const int nitems = hi - lo;                               // <= ROW_SLOTS (the host selects this pass only then)
     const int slot = (G >= 2) ? warp : (warp >> 1);
     const bool has = slot < nitems;
@@ -911,7 +956,7 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
     if (threadIdx.x < 2 * GE::ROW_SLOTS * HG) s_acc[threadIdx.x] = 0ull;
     if (has) {
         const int item = lo + slot;
-        const int b = (item * HG) / P.ny;
+        const int b = (item * HG) >> P.ny_log2;
         A = (f ? P.A[1] : P.A[0]) + (size_t)(item * HG + r) * NX;
         hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
@@ -926,7 +971,8 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
     // ---- phase B: point idx = ((local item) * HG + row in item) * NX + e; a warp's 32 points share a row
     const int total = nitems * HG * NX;
     const size_t plane = (size_t)P.ny * NX;
-    const TNode ta = t_node(n, P.nz, P.nzt), tb = t_node(n + 1, P.nz, P.nzt);
+    const TNode ta = sc.ta, tb = sc.tb;
+    const int rslot = sc.slot;
     for (int idx = threadIdx.x; idx < total; idx += GE::THREADS) {
         const int li = idx / (HG * NX), rr = (idx / NX) % HG, e = idx % NX;
         float2* l1;
@@ -941,7 +987,7 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
         float2* q1 = l1 + e;
         float2* q2 = l2 + ((e + NX / 2) & (NX - 1));
         const int row = (lo + li) * HG + rr;
-        const int b = row / P.ny, y = row - b * P.ny;
+        const int b = row >> P.ny_log2, y = row - (b << P.ny_log2);
         const MemberDev& mb = P.mem[b];
         const float k1dz = mb.kap1dz, k2dz = mb.kap2dz;
         PhaseCoef CA, CM, CB;
@@ -972,7 +1018,7 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
         *q1 = a1;
         *q2 = a2;
         // a warp's 32 points share a row: fixed-point warp sums into the row's shared accumulators
-        if (rec_slot(P, n + 1) >= 0) {
+        if (rslot >= 0) {
             const float fsc = P.pfix[b];
             const long long w1 = warp_sum_ll(to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc));
             const long long w2 = warp_sum_ll(to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc));
@@ -987,10 +1033,10 @@ __device__ __forceinline__ void row_pass_flat(const Params& P, int n, int hsel, 
     // ---- phase C: one thread per (row, field) adds the row's sum to the history (2 global atomics per row instead
     // of 2 per warp: they all hit the member's two history words, and the barrier's release waits for them)
     if ((int)threadIdx.x < nitems * HG * 2) {
-        const int slot = rec_slot(P, n + 1);
+        const int slot = rslot;
         if (slot >= 0) {
             const int row = lo * HG + (int)threadIdx.x / 2, fld = threadIdx.x & 1;
-            const int b = row / P.ny;
+            const int b = row >> P.ny_log2;
             fix_add(P.hfix + ((long long)b * (P.nrec + 1) + slot) * 2 + fld, (long long)s_acc[threadIdx.x]);
         }
     }
@@ -1018,12 +1064,11 @@ __device__ __forceinline__ void row_pass_paper(const Params& P, int n, float2* s
 }
 
 template <int NY, bool PREC, int NXC, bool TS = false>
-__device__ __forceinline__ void col_pass(const Params& P, int hsel, float2* smem_cta,
+__device__ __forceinline__ void col_pass(const Params& P, const StepCtx& sc, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
                                          const float4* __restrict__ stab = nullptr) {
     using GE = Geo<NY>;
-    int lo, hi;
-    cta_range(col_items<NY>(P.batch, P.nx), lo, hi);
+    const int lo = sc.col_lo, hi = sc.col_hi;
     const int team = warp / GE::TW, trank = warp % GE::TW;
     float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
     if (team >= P.col_teams) return;
@@ -1039,11 +1084,13 @@ __global__ void __launch_bounds__(Geo<NX>::THREADS, 1) k_row(Params P, int n, in
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     __shared__ unsigned long long s_pow[2];
+    __shared__ StepCtx sc;
     if (threadIdx.x < 2) s_pow[threadIdx.x] = 0ull;
+    if (threadIdx.x == 32) { ctx_rows<NX>(P, sc); ctx_step(P, sc, n); }
     const float4* tws = load_twiddles<NX>(smem_raw, P.twx);
     unsigned long long* sp = (MODE == ROW_MID && P.batch == 1) ? s_pow : nullptr;
-    row_pass<NX, MODE, PREC, HEAT>(P, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane, nullptr, sp);
-    if (sp) flush_powers(P, n, sp);
+    row_pass<NX, MODE, PREC, HEAT>(P, sc, n, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane, nullptr, sp);
+    if (sp) flush_powers(P, sc, sp);
 }
 
 template <int NX, int MODE, bool PREC>
@@ -1058,8 +1105,10 @@ template <int NY, bool PREC>
 __global__ void __launch_bounds__(Geo<NY>::THREADS, 1) k_col(Params P, int hsel) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ StepCtx sc;
+    if (threadIdx.x == 32) ctx_cols<NY>(P, sc);
     const float4* tws = load_twiddles<NY>(smem_raw, P.twy);
-    col_pass<NY, PREC, 0>(P, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
+    col_pass<NY, PREC, 0>(P, sc, hsel, reinterpret_cast<float2*>(smem_raw), tws, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1084,7 +1133,11 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
 // bar.sync, before the increment; no value returned, so no round trip), poll = relaxed loads (one L2 round
 // trip per poll; the timeout / status checks only every 32nd).  A bounded spin turns a lost CTA into an
 // error status instead of a hung GPU.
-__device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch, int n, int which) {
+// sc_next (barrier after a column pass): the polling thread fills in the step entries of z-step n + 1 between its
+// arrival and its first poll (every warp of the CTA is past its last read of the old entries: the opening
+// bar.sync), the closing bar.sync publishes them.
+__device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoch, int n, int which,
+                                             StepCtx* sc_next = nullptr) {
     __shared__ int ok;
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -1092,6 +1145,7 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         epoch += 1;
         const unsigned int target = epoch * gridDim.x;
         asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(P.barrier), "r"(1u) : "memory");
+        if (sc_next != nullptr && n + 1 < P.nz) ctx_step(P, *sc_next, n + 1);
         int good = 1;
         if (ld_relaxed_u32(P.barrier) < target) {
             const long long t0 = clock64();
@@ -1118,7 +1172,11 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         if (P.acquire_fence == 2) (void)ld_acquire_u32(P.barrier);
         else if (P.acquire_fence == 1) asm volatile("fence.acq_rel.gpu;" ::: "memory");
         ok = good;
+#ifdef SHG_WTRACE
+        if (P.trace != nullptr && n < (P.trace_steps < 200 ? P.trace_steps : 200)) {   // (the tail holds the warp stamps)
+#else
         if (P.trace != nullptr && n < P.trace_steps) {
+#endif
             long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
             unsigned long long gt;
             unsigned int smid;
@@ -1151,7 +1209,9 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
         }
     };
     __shared__ unsigned long long s_pow[2];
+    __shared__ StepCtx sc;
     if (threadIdx.x < 2) s_pow[threadIdx.x] = 0ull;
+    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, 0); }
     unsigned long long* sp = (P.batch == 1) ? s_pow : nullptr;
     __syncthreads();
     stage_tables(P.nz == 1 ? 1 : 0);
@@ -1160,11 +1220,11 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         if (hsel == 1 && n > 0) stage_tables(1);             // (every warp passed the barrier's closing bar.sync)
-        row_pass<N, ROW_MID, PREC, HEAT, TS>(P, n, hsel, smem_cta, tws, warp, lane, stab, sp);
-        if (sp) flush_powers(P, n, sp);
+        row_pass<N, ROW_MID, PREC, HEAT, TS>(P, sc, n, hsel, smem_cta, tws, warp, lane, stab, sp);
+        if (sp) flush_powers(P, sc, sp);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC, N, TS>(P, hsel, smem_cta, tws, warp, lane, stab);
-        if (!grid_barrier(P, epoch, n, 1)) return;
+        col_pass<N, PREC, N, TS>(P, sc, hsel, smem_cta, tws, warp, lane, stab);
+        if (!grid_barrier(P, epoch, n, 1, &sc)) return;
     }
 }
 
@@ -1174,16 +1234,18 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ unsigned long long s_acc[2 * Geo<N>::ROW_SLOTS * Geo<N>::HG];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ StepCtx sc;
+    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, 0); }
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
     unsigned int epoch = 0;
 #pragma unroll 1
     for (int n = 0; n < P.nz; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        row_pass_flat<N, PREC>(P, n, hsel, smem_cta, tws, warp, lane, s_acc);
+        row_pass_flat<N, PREC>(P, sc, n, hsel, smem_cta, tws, warp, lane, s_acc);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC, N>(P, hsel, smem_cta, tws, warp, lane);
-        if (!grid_barrier(P, epoch, n, 1)) return;
+        col_pass<N, PREC, N>(P, sc, hsel, smem_cta, tws, warp, lane);
+        if (!grid_barrier(P, epoch, n, 1, &sc)) return;
     }
 }
 
@@ -1193,6 +1255,8 @@ template <int N, bool PREC>
 __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_paper(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ StepCtx sc;
+    if (threadIdx.x == 32) ctx_cols<N>(P, sc);
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
     unsigned int epoch = 0;
@@ -1200,7 +1264,7 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_paper(Params P) 
     for (int n = 0; n < P.nz - 1; ++n) {
         row_pass_paper<N, ROW_MID, PREC>(P, n, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC, N>(P, 0, smem_cta, tws, warp, lane);
+        col_pass<N, PREC, N>(P, sc, 0, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1)) return;
     }
 }

@@ -21,6 +21,7 @@ struct MemberDev {
 
 struct Params {
     int nx, ny, nz, nzt, batch;
+    int ny_log2;               // ny = 1 << ny_log2 (every supported line length is a power of two)
     int flat_rows;             // 1: sparse launch, the persistent kernel spreads the nonlinear step over the CTA (row_pass_flat)
     int scheme;                // 0: L/2 - N - L/2 with merged half-steps; 1: the paper's N/2 - L - N/2 (SHG_OPT_SCHEME)
     int acquire_fence;         // acquire side of the device-wide barrier (SHG_OPT_ACQUIRE_FENCE): 0 none (L2-only loads),
