@@ -308,10 +308,16 @@ __device__ __forceinline__ void nl_rhs(float2 a1, float2 a2, const PhaseCoef& pc
     d1.y = fmaf(px, pc.u1y, py * pc.u1x);
     d2.x = fmaf(qx, pc.u2x, -qy * pc.u2y);
     d2.y = fmaf(qx, pc.u2y, qy * pc.u2x);
-    float t1 = -g1 * fmaf(a1.x, a1.x, a1.y * a1.y);
-    float t2 = -g2 * fmaf(a2.x, a2.x, a2.y * a2.y);
-    d1.x = fmaf(t1, a1.x, d1.x); d1.y = fmaf(t1, a1.y, d1.y);
-    d2.x = fmaf(t2, a2.x, d2.x); d2.y = fmaf(t2, a2.y, d2.y);
+    // (two-photon terms: g_j is the same for every point of a member, so the branches are warp-uniform; a term
+    // that is switched off -- beta_1 = 0 in every BASELINE config -- costs a predicate instead of five operations)
+    if (g1 != 0.f) {
+        float t1 = -g1 * fmaf(a1.x, a1.x, a1.y * a1.y);
+        d1.x = fmaf(t1, a1.x, d1.x); d1.y = fmaf(t1, a1.y, d1.y);
+    }
+    if (g2 != 0.f) {
+        float t2 = -g2 * fmaf(a2.x, a2.x, a2.y * a2.y);
+        d2.x = fmaf(t2, a2.x, d2.x); d2.y = fmaf(t2, a2.y, d2.y);
+    }
 }
 
 // One classical RK4 step of length dz; the phase is sampled at z_n, z_n + dz/2, z_n + dz (G8).
