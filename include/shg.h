@@ -123,6 +123,15 @@ typedef struct {
                                   cluster size whenever the grid size allows, even if the clusters run in several
                                   waves.  Same arithmetic as the other kernels: bit-identical fields and powers.   */
 
+#define SHG_OPT_PIPELINE   10   /* batched runs (batch >= 2) in the persistent kernel.  The members are split into
+                                  two groups whose row and column phases interleave, every device-wide barrier is
+                                  split-phase (arrive when a phase is done, wait one phase later), and no CTA-wide
+                                  barrier remains (k_persist_pipe): the barriers' latency and the skew between CTAs
+                                  stop nothing.  1 (default): when a warp has at least two row items per phase;
+                                  2: whenever batch >= 2; 0: never (one pair of device-wide barriers per z-step for
+                                  the whole batch, k_persist).  Not used with a heat output, SHG_OPT_SCHEME = 1 or
+                                  SHG_OPT_TRACE.  Same device code per row and strip: bit-identical results.      */
+
 /* beams: HOST array [grid->batch].  *out receives the context. */
 int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam* beams, shg_ctx** out);
 

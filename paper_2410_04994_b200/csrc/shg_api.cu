@@ -195,6 +195,7 @@ struct shg_ctx {
     int acquire_fence = 2;
     int tables_smem = 1;
     int cluster_mode = 1;                 // SHG_OPT_CLUSTER: 0 never, 1 auto, 8 / 16 that cluster size whenever possible
+    int pipeline = 1;                     // SHG_OPT_PIPELINE
     unsigned long long spin_limit = 4000000000ULL;
     int rec_every = 1, nrec = 0;
     bool undepleted = false;
@@ -217,7 +218,7 @@ struct shg_ctx {
     double* d_inpart = nullptr;          // k_input_power chunk sums [batch][64][2]
     unsigned int* d_ticket = nullptr;    // [batch]
     std::vector<double> pscale_in, pscale_step;   // [batch][2] (eps0 c n_j/2) dx dy, and times exp(-alpha_j dz/2)
-    unsigned int* d_barrier = nullptr;   // [0] barrier counter, [1] status word
+    unsigned int* d_barrier = nullptr;   // [0] barrier counter, [1] status word, [2..5] counters of the pipelined kernel
     float* d_T_owned = nullptr;
     float* d_Q = nullptr;              // borrowed heat-source output (shg_set_heat_output)
     int nq = 0;
@@ -476,7 +477,7 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     alloc((void**)&ctx->d_pfix, sizeof(float) * B);
     alloc((void**)&ctx->d_inpart, sizeof(double) * (size_t)B * 64 * 2);
     alloc((void**)&ctx->d_ticket, sizeof(unsigned int) * B);
-    alloc((void**)&ctx->d_barrier, 2 * sizeof(unsigned int));
+    alloc((void**)&ctx->d_barrier, 8 * sizeof(unsigned int));
     if (!ok) { free_ctx(ctx); return SHG_ECUDA; }
     e = cudaMemset(ctx->d_ticket, 0, sizeof(unsigned int) * B);
     if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaMemset"); }
@@ -507,6 +508,10 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
         case SHG_OPT_CLUSTER:
             if (value != 0 && value != 1 && value != 8 && value != 16) return SHG_EINVAL;
             ctx->cluster_mode = value;
+            return SHG_OK;
+        case SHG_OPT_PIPELINE:
+            if (value < 0 || value > 2) return SHG_EINVAL;
+            ctx->pipeline = value;
             return SHG_OK;
         case SHG_OPT_SCHEME:
             if (value != 0 && value != 1) return SHG_EINVAL;
@@ -648,7 +653,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const size_t np = np_of(ctx);
     int launches = 0;
     CU(cudaMemsetAsync(ctx->d_hfix, 0, sizeof(long long) * (size_t)g.batch * (ctx->nrec + 1) * 2, st));
-    CU(cudaMemsetAsync(ctx->d_barrier, 0, 2 * sizeof(unsigned int), st));
+    CU(cudaMemsetAsync(ctx->d_barrier, 0, 8 * sizeof(unsigned int), st));
     if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
     {   // P_j(0) and the fixed-point scale of every member, from the input (before anything overwrites it)
         int ch = (int)(np / 4096);
@@ -728,6 +733,15 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     }
     const bool prec = ctx->precise;
     P.tab_smem = (use_persist && ctx->tables_smem && batch == 1 && prec && ctx->scheme == 0 && !P.Q) ? 1 : 0;
+    {   // Batched runs: the software-pipelined kernel pays once a warp has a few row items per phase (two groups of
+        // members: half the items of a pass each); with less than two (cfg4: 0.9) a phase is one item per warp
+        // and the split only adds phases.  SHG_OPT_PIPELINE: 0 never, 1 auto (default), 2 whenever batch >= 2.
+        const int grid_p = grid_r > grid_c ? grid_r : grid_c;
+        const long long slots = (long long)grid_p * ix.row_slots;
+        const bool enough = ctx->pipeline == 2 || (long long)UR >= 4 * slots;
+        P.pipeline = (use_persist && ctx->pipeline != 0 && enough && batch >= 2 && ctx->scheme == 0 && !P.Q &&
+                      !P.trace) ? 1 : 0;
+    }
     {   // Sparse launch: every CTA owns at most one row item per slot and at most half of its warps have one
         // (single small simulations).  The persistent kernel then spreads the nonlinear step over the whole CTA.
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;

@@ -78,6 +78,18 @@ template <int N> struct Geo {
     // persistent kernel of a single simulation: the propagator tables hx, hy of both fields staged in shared memory
     static constexpr int TAB_SMEM = 4 * N * 16;            // [hx f=0][hx f=1][hy f=0][hy f=1], N float4 each
     static constexpr int CTA_SMEM_TAB = CTA_SMEM + TAB_SMEM;
+    // pipelined kernel (k_persist_pipe): no CTA-wide barrier separates a row pass from a column pass, so a team's strip
+    // must alias only the line regions of the team's own warps: one region per team, TEAM_SMEM bytes
+    static constexpr int TEAM_SMEM = ((TW * WARP_SMEM > STRIP_SMEM ? TW * WARP_SMEM : STRIP_SMEM) + 15) / 16 * 16;
+    static constexpr int PIPE_WORK_SMEM = TEAMS * TEAM_SMEM;
+    static constexpr int PIPE_SMEM = PIPE_WORK_SMEM + TW_SMEM;
+    static_assert(PIPE_SMEM <= 227 * 1024 && (TEAM_SMEM - TW * WARP_SMEM) % 8 == 0, "pipelined kernel: shared memory");
+    // ... and, where it fits (N <= 256), one staging buffer per warp (the G lines of a row item) and per team (the
+    // strip, [N][SC] dense) that the NEXT item's input is copied into asynchronously while this item is computed
+    static constexpr bool STAGE = (N <= 256);
+    static constexpr int ROW_STAGE_SMEM = WARPS * G * N * 8, COL_STAGE_SMEM = TEAMS * N * SC * 8;
+    static constexpr int PIPE_SMEM_STG = PIPE_SMEM + (STAGE ? ROW_STAGE_SMEM + COL_STAGE_SMEM : 0);
+    static_assert(PIPE_SMEM_STG <= 227 * 1024, "pipelined kernel: staging buffers");
     static_assert(CTA_SMEM_TAB <= 227 * 1024, "shared memory budget");
     static_assert(WARPS % TW == 0 && WARPS % 2 == 0, "team / pair layout");
     static_assert(TEAMS + 1 <= 16 && WARPS / 2 + 1 <= 16, "named barrier ids");
@@ -89,6 +101,13 @@ __device__ __forceinline__ void stcg2(float2* p, float2 v) { __stcg(p, v); }
 __device__ __forceinline__ void named_barrier(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+
+// 16-byte asynchronous copy global -> shared (LDGSTS, L2 only), completion with cp.async.wait_all
+__device__ __forceinline__ void cp_async16(float2* dst_smem, const float2* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
+                 ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // Table loads whose address carries a (numerically void) dependency on an earlier result.  Without it ptxas
 // hoists all R twiddle / propagator loads (4 registers each) far above their use and spills the line data
@@ -413,11 +432,27 @@ __device__ __forceinline__ void ctx_step(const Params& P, StepCtx& sc, int n) {
 // ------------------------------------------------------------------------------------------------
 // HEAT: also write the heat source of Eq. 8 (a separate instantiation: the common path carries none of it).
 // TS: the hx tables are read from shared memory (stab: [2][NX] float4, single simulation) instead of global / L1.
-template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
+// The G lines of row item `item` (both fields of HG rows) into a warp's staging buffer [G][NX], asynchronously.
+template <int NX>
+__device__ __forceinline__ void row_prefetch(const Params& P, int item, float2* stg, int lane) {
+    using GE = Geo<NX>;
+    constexpr int CH = NX / 2;                                // 16-byte chunks per line
+#pragma unroll
+    for (int c = lane; c < GE::G * CH; c += 32) {
+        const int gl = c / CH, ch = c % CH;                   // line gl = f * HG + r
+        const float2* src = (gl / GE::HG ? P.A[1] : P.A[0]) + (size_t)(item * GE::HG + gl % GE::HG) * NX + 2 * ch;
+        cp_async16(stg + gl * NX + 2 * ch, src);
+    }
+}
+
+// STG (k_persist_pipe, N <= 256): the item's input was copied into the warp's staging buffer `stg` by an asynchronous
+// copy issued one item earlier; this item issues the copy of item `next` (< 0: none) as soon as its own values are
+// in registers, so the load latency (L2 / HBM) of an item runs under the arithmetic of the previous one.
+template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false, bool STG = false>
 __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int item, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
                                          const float4* __restrict__ stab = nullptr,
-                                         unsigned long long* s_pow = nullptr) {
+                                         unsigned long long* s_pow = nullptr, float2* stg = nullptr, int next = -1) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
     const int g = lane / M, m = lane % M;
@@ -469,8 +504,17 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
         SHG_WT(0);
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
         const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
+        if constexpr (STG) {
+            cp_async_wait_all();
+            __syncwarp();
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+            for (int q = 0; q < R; ++q) v[q] = stg[g * NX + M * q + m];
+            __syncwarp();
+            if (next >= 0) row_prefetch<NX>(P, next, stg, lane);
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
+        }
         if constexpr (!TS) table_prefetch<R, M>(hx, m);
         if (P.nzt == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.ucoef + ((size_t)b * P.nz + n) * 3));
         // temperature / phase operands of the first RK4 point are requested before the transform (when
@@ -850,10 +894,24 @@ __device__ __forceinline__ void tile_fft(float2 (&v)[FftCfg<N>::R], float2* __re
 // ------------------------------------------------------------------------------------------------
 // NXC: the row length when it is known at compile time (square grids in the persistent kernel: every
 // load / store is then one base register plus an immediate), 0 = take P.nx.
-template <int NY, bool PREC, int NXC, bool TS = false>
+// The strip of column item `item` ([NY] rows x 64 B) into a team's staging buffer [NY][SC], asynchronously.
+template <int NY, int NXC>
+__device__ __forceinline__ void col_prefetch(const Params& P, int item, float2* cstg, int trank, int lane) {
+    using GE = Geo<NY>;
+    const int nx = NXC ? NXC : P.nx;
+    const int spf = nx / GE::SC;
+    const int bf = item / spf;
+    const float2* A = P.A[bf & 1] + (size_t)(bf >> 1) * NY * nx + (item - bf * spf) * GE::SC;
+#pragma unroll
+    for (int c = trank * 32 + lane; c < 4 * NY; c += GE::TW * 32)
+        cp_async16(cstg + (c >> 2) * GE::SC + 2 * (c & 3), A + (size_t)(c >> 2) * nx + 2 * (c & 3));
+}
+
+template <int NY, bool PREC, int NXC, bool TS = false, bool STG = false>
 __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, float2* strip,
                                          const float4* __restrict__ tws, int trank, int bar_id, int lane,
-                                         const float4* __restrict__ stab = nullptr) {
+                                         const float4* __restrict__ stab = nullptr, float2* cstg = nullptr,
+                                         int next = -1) {
     using GE = Geo<NY>;
     constexpr int R = GE::R, M = GE::M, SC = GE::SC, CP = GE::CP;
     static_assert(SC == 8 && GE::TW * 4 == M, "tile layout: 8 columns x 4 residues per warp");
@@ -868,8 +926,18 @@ __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, fl
     float2* colline = strip + c * CP;
     float2 v[R];
 
+    if constexpr (STG) {
+        // (see row_item: the strip was staged one item earlier by all threads of the team)
+        cp_async_wait_all();
+        named_barrier(bar_id, GE::TW * 32);
 #pragma unroll
-    for (int q = 0; q < R; ++q) v[q] = ldcg2(A + q * gstep);
+        for (int q = 0; q < R; ++q) v[q] = cstg[(t + M * q) * SC + c];
+        named_barrier(bar_id, GE::TW * 32);
+        if (next >= 0) col_prefetch<NY, NXC>(P, next, cstg, trank, lane);
+    } else {
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + q * gstep);
+    }
     if constexpr (!TS) table_prefetch<R, M>(h, t);
     tile_fft<NY, PREC>(v, colline, tws, t, bar_id);
     if constexpr (TS)      // (single simulation: bf is the field; the hy tables follow the two hx tables)
@@ -1252,6 +1320,162 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
         if (!grid_barrier(P, epoch, n, 0)) return;
         col_pass<N, PREC, N>(P, sc, hsel, smem_cta, tws, warp, lane);
         if (!grid_barrier(P, epoch, n, 1, &sc)) return;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Persistent kernel for BATCHED runs (batch >= 2), software pipelined over two groups of members.
+//
+// The members of a batch are independent simulations (the paper sweeps parameters by running one simulation
+// per process); only the rows and columns of ONE member depend on each other.  k_persist nevertheless stops the
+// whole device twice per z-step: ncu on cfg4 (64 x 128 x 128) shows 27 % of the warp-time parked at barriers -- the
+// ~1.9 K clocks of the barrier itself plus the skew between CTAs and between the warps of a CTA, in a pass of only
+// 3.5 items per warp.  Here the members are split into two groups with their own device-wide barriers, and every
+// barrier is SPLIT-PHASE: a warp arrives when its items of a phase are done and waits only before the first
+// access that needs the other CTAs' results -- one whole phase of the other group later:
+//
+//     wait C0 | rows of group 0 | arrive R0 | wait C1 | rows of group 1 | arrive R1 |
+//     wait R0 | cols of group 0 | arrive C0 | wait R1 | cols of group 1 | arrive C1 |      (one z-step)
+//
+// so a barrier is normally complete when a warp asks, and neither its latency nor the skew stops anything.  There
+// is no CTA-wide barrier either: warps, warp pairs and teams run through the phases on their own.
+//   arrive: __syncwarp, lane 0 adds 1 to the CTA's shared counter of that barrier (atom.acq_rel.cta); the warp that
+//           completes the CTA's count adds 1 to the device counter (red.release.gpu) -- cumulativity makes every
+//           warp's stores visible with it.
+//   wait:   lane 0 looks at the CTA's cached copy of the device counter (ld.acquire.cta, shared memory), else polls
+//           the device counter (relaxed, then one ld.acquire.gpu) and publishes the value (atom.max.release.cta);
+//           __syncwarp carries the ordering to the warp.
+// Shared memory: one region per team (Geo::TEAM_SMEM) holds the lines of the team's warps in a row phase and the
+// team's strip in a column phase.  Items are dealt to the slots round robin CONTINUING from phase to phase, so the
+// per-warp work of a z-step stays even although a phase has only a few items per slot.
+// Same device code per item as k_persist / k_row / k_col: bit-identical fields and powers.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned ld_acquire_cta_shared(unsigned saddr) {
+    unsigned v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+
+// counters: gcnt[k] device-wide (one arrival per CTA and instance), s_cnt[k] / s_seen[k] per CTA
+__device__ __forceinline__ void pipe_arrive(unsigned int* gcnt, unsigned int* s_cnt, int lane) {
+    __syncwarp();
+    if (lane == 0) {
+        unsigned old;
+        asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;"
+                     : "=r"(old) : "r"((unsigned)__cvta_generic_to_shared(s_cnt)) : "memory");
+        // (an instance's arrivals begin only after the previous instance of the same barrier completed)
+        if ((old + 1) % (blockDim.x >> 5) == 0)
+            asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(gcnt), "r"(1u) : "memory");
+    }
+}
+
+// (a wait that times out raises the status word and lets the warp run on with invalid data: every warp keeps the
+// same control flow, so no team or pair barrier is left hanging, and every later wait gives up at its first check)
+__device__ __forceinline__ void pipe_wait(const Params& P, const unsigned int* gcnt, unsigned int* s_seen,
+                                          unsigned int target, int lane) {
+    if (lane == 0) {
+        int good = 1;
+        const unsigned sa = (unsigned)__cvta_generic_to_shared(s_seen);
+        if (ld_acquire_cta_shared(sa) < target) {
+            unsigned v = ld_relaxed_u32(gcnt);
+            if (v < target) {
+                const long long t0 = clock64();
+                int spins = 0;
+                while ((v = ld_relaxed_u32(gcnt)) < target) {
+                    if (((spins++) & 31) == 0) {
+                        if (P.spin_limit != 0 && (unsigned long long)(clock64() - t0) > P.spin_limit) {
+                            good = 0; atomicExch(P.status, 1); break;
+                        }
+                        if (*((volatile int*)P.status) != 0) { good = 0; break; }
+                    }
+                }
+            }
+            if (good) {
+                v = ld_acquire_u32(gcnt);
+                asm volatile("atom.release.cta.shared.max.u32 %0, [%1], %2;" : "=r"(v) : "r"(sa), "r"(v) : "memory");
+            }
+        }
+    }
+    __syncwarp();                                   // carries the ordering to the other lanes
+}
+
+template <int N, bool PREC>
+__global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_pipe(Params P) {
+    using GE = Geo<N>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ unsigned int s_cnt[4], s_seen[4];
+    __shared__ int s_rng[2][4];                              // per group: row lo, row hi, col lo, col hi
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float4* twsw = reinterpret_cast<float4*>(smem_raw + GE::PIPE_WORK_SMEM);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) twsw[i] = P.twx[i];     // twx == twy on a square grid
+    if (threadIdx.x < 4) { s_cnt[threadIdx.x] = 0u; s_seen[threadIdx.x] = 0u; }
+    const int B0 = (P.batch + 1) / 2;                        // members of group 0; group 1 takes the rest
+    if (threadIdx.x < 2) {
+        const int g = threadIdx.x;
+        const int m0 = g ? B0 : 0, m1 = g ? P.batch : B0;
+        const int rpm = P.ny / GE::HG, cpm = 2 * (N / GE::SC);                // row items / strips per member
+        int lo, hi;
+        cta_range((m1 - m0) * rpm, lo, hi);
+        s_rng[g][0] = m0 * rpm + lo; s_rng[g][1] = m0 * rpm + hi;
+        cta_range((m1 - m0) * cpm, lo, hi);
+        s_rng[g][2] = m0 * cpm + lo; s_rng[g][3] = m0 * cpm + hi;
+    }
+    __syncthreads();
+    const float4* tws = twsw;
+    const int team = warp / GE::TW, trank = warp % GE::TW;
+    // row items address their lines as base + warp * WARP_SMEM: shift the base so that they fall into the team's region
+    float2* row_base = reinterpret_cast<float2*>(smem_raw + (size_t)team * (GE::TEAM_SMEM - GE::TW * GE::WARP_SMEM));
+    float2* strip = reinterpret_cast<float2*>(smem_raw + (size_t)team * GE::TEAM_SMEM);
+    constexpr bool STG = GE::STAGE;
+    float2* rstg = reinterpret_cast<float2*>(smem_raw + GE::PIPE_SMEM) + (size_t)warp * (GE::G * N);
+    float2* cstg = reinterpret_cast<float2*>(smem_raw + GE::PIPE_SMEM + GE::ROW_STAGE_SMEM) + (size_t)team * (N * GE::SC);
+    const int rslot = (GE::G >= 2) ? warp : (warp >> 1);
+    // named barriers: warp pairs of a row phase use 1 + pair (G == 1), teams of a column phase 9 + team then
+    // (pairs and teams of different phases run at the same time)
+    const int bar_id = (GE::G == 1 ? 9 : 1) + team;
+    static_assert(GE::G == 1 ? GE::TEAMS <= 7 : GE::TEAMS <= 15, "named barrier ids");
+    // barriers: 0 = R0, 1 = R1 (rows of group g done), 2 = C0, 3 = C1 (columns of group g done)
+    unsigned int* gcnt = P.barrier + 2;
+    // where the round-robin deal of each kind of item stands (continues over phases and z-steps)
+    int rdeal = 0, cdeal = 0;
+    StepCtx sc;
+#pragma unroll 1
+    for (int n = 0; n < P.nz; ++n) {
+        const int hsel = (n == P.nz - 1) ? 1 : 0;
+        sc.ta = t_node(n, P.nz, P.nzt);
+        sc.tb = t_node(n + 1, P.nz, P.nzt);
+        sc.slot = rec_slot(P, n + 1);
+#pragma unroll 1
+        for (int g = 0; g < 2; ++g) {
+            // the columns of this group's previous z-step are complete everywhere (n = 0: the launch boundary)
+            if (n > 0) pipe_wait(P, gcnt + 2 + g, &s_seen[2 + g], (unsigned)n * gridDim.x, lane);
+            const int lo = s_rng[g][0], hi = s_rng[g][1];
+            // item lo + i goes to slot (rdeal + i) % ROW_SLOTS
+            int i = (rslot - rdeal % GE::ROW_SLOTS + GE::ROW_SLOTS) % GE::ROW_SLOTS;
+            if constexpr (STG) { if (lo + i < hi) row_prefetch<N>(P, lo + i, rstg, lane); }
+            for (; lo + i < hi; i += GE::ROW_SLOTS)
+                row_item<N, ROW_MID, PREC, false, false, STG>(P, sc, lo + i, n, hsel, row_base, tws, warp, lane, nullptr,
+                                                              nullptr, rstg, lo + i + GE::ROW_SLOTS < hi ? lo + i + GE::ROW_SLOTS : -1);
+            rdeal += hi - lo;
+            pipe_arrive(gcnt + g, &s_cnt[g], lane);
+        }
+#pragma unroll 1
+        for (int g = 0; g < 2; ++g) {
+            pipe_wait(P, gcnt + g, &s_seen[g], (unsigned)(n + 1) * gridDim.x, lane);
+            const int lo = s_rng[g][2], hi = s_rng[g][3];
+            bool any = false;
+            int i = (team - cdeal % GE::TEAMS + GE::TEAMS) % GE::TEAMS;
+            if constexpr (STG) { if (lo + i < hi) col_prefetch<N, N>(P, lo + i, cstg, trank, lane); }
+            for (; lo + i < hi; i += GE::TEAMS) {
+                col_item<N, PREC, N, false, STG>(P, lo + i, hsel, strip, tws, trank, bar_id, lane, nullptr, cstg,
+                                                 lo + i + GE::TEAMS < hi ? lo + i + GE::TEAMS : -1);
+                any = true;
+            }
+            // the team's region turns into line buffers again: every warp of the team is done reading the strip
+            if (any) named_barrier(bar_id, GE::TW * 32);
+            cdeal += hi - lo;
+            pipe_arrive(gcnt + 2 + g, &s_cnt[2 + g], lane);
+        }
     }
 }
 

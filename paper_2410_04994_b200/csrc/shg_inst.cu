@@ -107,6 +107,15 @@ cudaError_t SHG_CAT(launch_persist_, SHG_N)(const Params& P, bool prec, int grid
         void* args[] = {&Pc};
         return cudaLaunchCooperativeKernel(kf, dim3(grid), dim3(GE::THREADS), args, (size_t)smem, st);
     }
+    if (P.pipeline) {
+        const int smem = GE::PIPE_SMEM_STG;
+        const void* kf = prec ? (const void*)k_persist_pipe<N, true> : (const void*)k_persist_pipe<N, false>;
+        cudaError_t e = cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        Params Pc = P;
+        void* args[] = {&Pc};
+        return cudaLaunchCooperativeKernel(kf, dim3(grid), dim3(GE::THREADS), args, (size_t)smem, st);
+    }
     if (P.Q) return prec ? launch_persist_t<true, true>(P, grid, st) : launch_persist_t<false, true>(P, grid, st);
     if (P.tab_smem && prec) return launch_persist_t<true, false, true>(P, grid, st);
     return prec ? launch_persist_t<true, false>(P, grid, st) : launch_persist_t<false, false>(P, grid, st);

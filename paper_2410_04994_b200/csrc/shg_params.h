@@ -26,6 +26,7 @@ struct Params {
     int scheme;                // 0: L/2 - N - L/2 with merged half-steps; 1: the paper's N/2 - L - N/2 (SHG_OPT_SCHEME)
     int acquire_fence;         // acquire side of the device-wide barrier (SHG_OPT_ACQUIRE_FENCE): 0 none (L2-only loads),
                                // 1 gpu-scope fence after the poll, 2 the successful poll is an ld.acquire.gpu
+    int pipeline;              // 1: batched run in the software-pipelined persistent kernel (k_persist_pipe)
     int tab_smem;              // 1: the propagator tables hx / hy of member 0 are staged in shared memory (batch == 1)
     int rec_every, nrec;       // power history: nodes n with n % rec_every == 0, and node nz (slot nrec), are recorded
     unsigned long long spin_limit;   // device-wide barrier: SM clocks before a timeout is declared (0 = wait forever)
@@ -46,7 +47,7 @@ struct Params {
     float* Q;                  // optional heat-source output [batch][nq][ny][nx] (shg_set_heat_output), else null
     const int* qmap;           // [nz]: plane of Q that samples z-step n, or -1
     int nq;
-    unsigned int* barrier;     // grid barrier counter (persistent kernel)
+    unsigned int* barrier;     // grid barrier counter (persistent kernel); [2..5]: the four counters of k_persist_pipe
     int* status;               // device status word (barrier timeout)
     long long* trace;          // optional phase timeline of the persistent kernel (SHG_OPT_TRACE), else null:
     int trace_steps;           //   [trace_steps][grid][2 barriers][4] = {clock64 CTA done, clock64 grid done, globaltimer, smid}

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libshg.so")
 
 SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
 OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE, OPT_UNDEPLETED, OPT_SCHEME = 1, 2, 3, 4, 5, 6
-OPT_SPIN_LIMIT, OPT_TABLES_SMEM, OPT_CLUSTER = 7, 8, 9
+OPT_SPIN_LIMIT, OPT_TABLES_SMEM, OPT_CLUSTER, OPT_PIPELINE = 7, 8, 9, 10
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",

@@ -301,6 +301,38 @@ def test_batch_with_per_member_temperature_and_partial_batch():
     assert ei.value.code == shg.SHG_ESTATE
 
 
+@pytest.mark.parametrize("n,B,nz,nzt", [(128, 5, 9, 4), (64, 40, 7, 0), (256, 7, 6, 7), (1024, 2, 5, 3), (1024, 3, 4, 0),
+                                        (512, 2, 3, 1)])
+def test_pipelined_batched_kernel_gives_the_same_bits(n, B, nz, nzt):
+    """SHG_OPT_PIPELINE (k_persist_pipe: two groups of members, split-phase device-wide barriers, no CTA-wide
+    barrier) runs the same device code per row and strip as k_persist and the per-pass launches: fields and power
+    history of every member identical bit for bit -- odd batches, per-member temperature arrays, uniform
+    temperature, warp pairs (1024) and warp groups, the last z-step's half-step tables."""
+    c = wl.crystal(5e-3, alpha=True, ddk_dT=-400.0)
+    beams = [wl.beam(c, 60.0 * (b % 7 + 1), 0.5 + 0.13 * (b % 11), 6.0) for b in range(B)]
+    rng = np.random.default_rng(11 + n)
+    T = (wl.T_PM + rng.uniform(0, 3, (B, nzt, n, n))).astype(np.float32) if nzt else None
+    A1 = np.stack([wl.gaussian_pump(n, n, c, bm) for bm in beams])
+    A2 = (0.05 * np.abs(A1).max() * (rng.standard_normal(A1.shape) + 1j * rng.standard_normal(A1.shape))).astype(np.complex64)
+    w = dict(grid=dict(nx=n, ny=n, nz=nz, nzt=nzt, batch=B), crystal=c, beams=beams, T=T, T_uniform=wl.T_PM + 0.7,
+             per_member=bool(nzt), A1=A1)
+    base = {shg.OPT_CLUSTER: 0, shg.OPT_PIPELINE: 2}
+    p1, p2, ph, cp = run_gpu(w, A2=A2, options=base)
+    assert cp.last_launch_count() == 5
+    q1, q2, qh, cq = run_gpu(w, A2=A2, options={shg.OPT_CLUSTER: 0, shg.OPT_PIPELINE: 0})
+    assert cq.last_launch_count() == 5
+    r1, r2, rh, cr = run_gpu(w, A2=A2, options=base, persistent=False)
+    assert cr.last_launch_count() == 4 + 2 * nz
+    for a1, a2, ah in ((q1, q2, qh), (r1, r2, rh)):
+        assert np.array_equal(p1, a1) and np.array_equal(p2, a2)
+        assert all(np.array_equal(ph[b], ah[b]) for b in range(B))
+    assert np.isfinite(p1).all() and np.abs(p2).max() > 0
+    # a second propagate on the same context (counters reset, same bits)
+    s1, s2 = cp.propagate(torch.from_numpy(A1).cuda(), torch.from_numpy(A2).cuda())
+    torch.cuda.synchronize()
+    assert np.array_equal(s1.cpu().numpy(), p1) and np.array_equal(s2.cpu().numpy(), p2)
+
+
 def test_free_diffraction_matches_analytic_beam_on_gpu():
     """d_eff = 0: the GPU linear path alone against Eq. 5, no oracle involved."""
     n = 256
