@@ -84,11 +84,13 @@ template <int N> struct Geo {
     static constexpr int PIPE_WORK_SMEM = TEAMS * TEAM_SMEM;
     static constexpr int PIPE_SMEM = PIPE_WORK_SMEM + TW_SMEM;
     static_assert(PIPE_SMEM <= 227 * 1024 && (TEAM_SMEM - TW * WARP_SMEM) % 8 == 0, "pipelined kernel: shared memory");
-    // ... and, where it fits (N <= 256), one staging buffer per warp (the G lines of a row item) and per team (the
-    // strip, [N][SC] dense) that the NEXT item's input is copied into asynchronously while this item is computed
-    static constexpr bool STAGE = (N <= 256);
-    static constexpr int ROW_STAGE_SMEM = WARPS * G * N * 8, COL_STAGE_SMEM = TEAMS * N * SC * 8;
-    static constexpr int PIPE_SMEM_STG = PIPE_SMEM + (STAGE ? ROW_STAGE_SMEM + COL_STAGE_SMEM : 0);
+    // ... and, where it fits (N <= 256), one staging buffer per team ([N][SC] dense) that the NEXT strip is copied into
+    // asynchronously while this one is transformed.  (The same for the lines of a row item was measured slower:
+    // stream256 271 us per z-step against 255 with the strips alone -- it costs 64 KB of L1, through which the
+    // batched kernels read their propagator tables, and the row items' 8-byte loads were not the problem.)
+    static constexpr bool STAGE_COL = (N <= 256);
+    static constexpr int COL_STAGE_SMEM = STAGE_COL ? TEAMS * N * SC * 8 : 0;
+    static constexpr int PIPE_SMEM_STG = PIPE_SMEM + COL_STAGE_SMEM;
     static_assert(PIPE_SMEM_STG <= 227 * 1024, "pipelined kernel: staging buffers");
     static_assert(CTA_SMEM_TAB <= 227 * 1024, "shared memory budget");
     static_assert(WARPS % TW == 0 && WARPS % 2 == 0, "team / pair layout");
@@ -432,27 +434,11 @@ __device__ __forceinline__ void ctx_step(const Params& P, StepCtx& sc, int n) {
 // ------------------------------------------------------------------------------------------------
 // HEAT: also write the heat source of Eq. 8 (a separate instantiation: the common path carries none of it).
 // TS: the hx tables are read from shared memory (stab: [2][NX] float4, single simulation) instead of global / L1.
-// The G lines of row item `item` (both fields of HG rows) into a warp's staging buffer [G][NX], asynchronously.
-template <int NX>
-__device__ __forceinline__ void row_prefetch(const Params& P, int item, float2* stg, int lane) {
-    using GE = Geo<NX>;
-    constexpr int CH = NX / 2;                                // 16-byte chunks per line
-#pragma unroll
-    for (int c = lane; c < GE::G * CH; c += 32) {
-        const int gl = c / CH, ch = c % CH;                   // line gl = f * HG + r
-        const float2* src = (gl / GE::HG ? P.A[1] : P.A[0]) + (size_t)(item * GE::HG + gl % GE::HG) * NX + 2 * ch;
-        cp_async16(stg + gl * NX + 2 * ch, src);
-    }
-}
-
-// STG (k_persist_pipe, N <= 256): the item's input was copied into the warp's staging buffer `stg` by an asynchronous
-// copy issued one item earlier; this item issues the copy of item `next` (< 0: none) as soon as its own values are
-// in registers, so the load latency (L2 / HBM) of an item runs under the arithmetic of the previous one.
-template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false, bool STG = false>
+template <int NX, int MODE, bool PREC, bool HEAT = false, bool TS = false>
 __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int item, int n, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
                                          const float4* __restrict__ stab = nullptr,
-                                         unsigned long long* s_pow = nullptr, float2* stg = nullptr, int next = -1) {
+                                         unsigned long long* s_pow = nullptr) {
     using GE = Geo<NX>;
     constexpr int R = GE::R, M = GE::M, G = GE::G, NP = GE::NP, HG = GE::HG, H = R / 2;
     const int g = lane / M, m = lane % M;
@@ -504,17 +490,8 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
         SHG_WT(0);
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
         const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
-        if constexpr (STG) {
-            cp_async_wait_all();
-            __syncwarp();
 #pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = stg[g * NX + M * q + m];
-            __syncwarp();
-            if (next >= 0) row_prefetch<NX>(P, next, stg, lane);
-        } else {
-#pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
-        }
+        for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
         if constexpr (!TS) table_prefetch<R, M>(hx, m);
         if (P.nzt == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.ucoef + ((size_t)b * P.nz + n) * 3));
         // temperature / phase operands of the first RK4 point are requested before the transform (when
@@ -927,7 +904,9 @@ __device__ __forceinline__ void col_item(const Params& P, int item, int hsel, fl
     float2 v[R];
 
     if constexpr (STG) {
-        // (see row_item: the strip was staged one item earlier by all threads of the team)
+        // the strip was copied into the team's staging buffer one item earlier (all threads of the team); the copy of
+        // strip `next` (< 0: none) is issued as soon as this one is in registers, so its L2 / HBM latency runs under
+        // this strip's transforms
         cp_async_wait_all();
         named_barrier(bar_id, GE::TW * 32);
 #pragma unroll
@@ -1137,17 +1116,28 @@ __device__ __forceinline__ void row_pass_paper(const Params& P, int n, float2* s
         row_item_paper<NX, MODE, PREC>(P, it, n, smem_cta, tws, warp, lane);
 }
 
-template <int NY, bool PREC, int NXC, bool TS = false>
+// CS: the team stages its next strip asynchronously while it transforms this one (cstg_cta: the staging buffers,
+// [TEAMS][NY][SC]; see col_item)
+template <int NY, bool PREC, int NXC, bool TS = false, bool CS = false>
 __device__ __forceinline__ void col_pass(const Params& P, const StepCtx& sc, int hsel, float2* smem_cta,
                                          const float4* __restrict__ tws, int warp, int lane,
-                                         const float4* __restrict__ stab = nullptr) {
+                                         const float4* __restrict__ stab = nullptr, float2* cstg_cta = nullptr) {
     using GE = Geo<NY>;
     const int lo = sc.col_lo, hi = sc.col_hi;
     const int team = warp / GE::TW, trank = warp % GE::TW;
     float2* strip = smem_cta + (size_t)team * (GE::SC * GE::CP);
     if (team >= P.col_teams) return;
-    for (int it = lo + team; it < hi; it += P.col_teams)
-        col_item<NY, PREC, NXC, TS>(P, it, hsel, strip, tws, trank, 1 + team, lane, stab);
+    if constexpr (CS) {
+        float2* cstg = cstg_cta + (size_t)team * (NY * GE::SC);
+        int it = lo + team;
+        if (it < hi) col_prefetch<NY, NXC>(P, it, cstg, trank, lane);
+        for (; it < hi; it += P.col_teams)
+            col_item<NY, PREC, NXC, TS, true>(P, it, hsel, strip, tws, trank, 1 + team, lane, stab, cstg,
+                                              it + P.col_teams < hi ? it + P.col_teams : -1);
+    } else {
+        for (int it = lo + team; it < hi; it += P.col_teams)
+            col_item<NY, PREC, NXC, TS>(P, it, hsel, strip, tws, trank, 1 + team, lane, stab);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1297,7 +1287,10 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
         row_pass<N, ROW_MID, PREC, HEAT, TS>(P, sc, n, hsel, smem_cta, tws, warp, lane, stab, sp);
         if (sp) flush_powers(P, sc, sp);
         if (!grid_barrier(P, epoch, n, 0)) return;
-        col_pass<N, PREC, N, TS>(P, sc, hsel, smem_cta, tws, warp, lane, stab);
+        // (batched runs, N <= 256: a team's next strip is staged under the transforms of this one)
+        constexpr bool CS = !TS && !HEAT && Geo<N>::STAGE_COL;
+        col_pass<N, PREC, N, TS, CS>(P, sc, hsel, smem_cta, tws, warp, lane, stab,
+                                     reinterpret_cast<float2*>(smem_raw + Geo<N>::CTA_SMEM));
         if (!grid_barrier(P, epoch, n, 1, &sc)) return;
     }
 }
@@ -1426,9 +1419,8 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_pipe(Params P) {
     // row items address their lines as base + warp * WARP_SMEM: shift the base so that they fall into the team's region
     float2* row_base = reinterpret_cast<float2*>(smem_raw + (size_t)team * (GE::TEAM_SMEM - GE::TW * GE::WARP_SMEM));
     float2* strip = reinterpret_cast<float2*>(smem_raw + (size_t)team * GE::TEAM_SMEM);
-    constexpr bool STG = GE::STAGE;
-    float2* rstg = reinterpret_cast<float2*>(smem_raw + GE::PIPE_SMEM) + (size_t)warp * (GE::G * N);
-    float2* cstg = reinterpret_cast<float2*>(smem_raw + GE::PIPE_SMEM + GE::ROW_STAGE_SMEM) + (size_t)team * (N * GE::SC);
+    constexpr bool CSTG = GE::STAGE_COL;
+    float2* cstg = reinterpret_cast<float2*>(smem_raw + GE::PIPE_SMEM) + (size_t)team * (N * GE::SC);
     const int rslot = (GE::G >= 2) ? warp : (warp >> 1);
     // named barriers: warp pairs of a row phase use 1 + pair (G == 1), teams of a column phase 9 + team then
     // (pairs and teams of different phases run at the same time)
@@ -1451,11 +1443,8 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_pipe(Params P) {
             if (n > 0) pipe_wait(P, gcnt + 2 + g, &s_seen[2 + g], (unsigned)n * gridDim.x, lane);
             const int lo = s_rng[g][0], hi = s_rng[g][1];
             // item lo + i goes to slot (rdeal + i) % ROW_SLOTS
-            int i = (rslot - rdeal % GE::ROW_SLOTS + GE::ROW_SLOTS) % GE::ROW_SLOTS;
-            if constexpr (STG) { if (lo + i < hi) row_prefetch<N>(P, lo + i, rstg, lane); }
-            for (; lo + i < hi; i += GE::ROW_SLOTS)
-                row_item<N, ROW_MID, PREC, false, false, STG>(P, sc, lo + i, n, hsel, row_base, tws, warp, lane, nullptr,
-                                                              nullptr, rstg, lo + i + GE::ROW_SLOTS < hi ? lo + i + GE::ROW_SLOTS : -1);
+            for (int i = (rslot - rdeal % GE::ROW_SLOTS + GE::ROW_SLOTS) % GE::ROW_SLOTS; lo + i < hi; i += GE::ROW_SLOTS)
+                row_item<N, ROW_MID, PREC>(P, sc, lo + i, n, hsel, row_base, tws, warp, lane);
             rdeal += hi - lo;
             pipe_arrive(gcnt + g, &s_cnt[g], lane);
         }
@@ -1465,9 +1454,9 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_pipe(Params P) {
             const int lo = s_rng[g][2], hi = s_rng[g][3];
             bool any = false;
             int i = (team - cdeal % GE::TEAMS + GE::TEAMS) % GE::TEAMS;
-            if constexpr (STG) { if (lo + i < hi) col_prefetch<N, N>(P, lo + i, cstg, trank, lane); }
+            if constexpr (CSTG) { if (lo + i < hi) col_prefetch<N, N>(P, lo + i, cstg, trank, lane); }
             for (; lo + i < hi; i += GE::TEAMS) {
-                col_item<N, PREC, N, false, STG>(P, lo + i, hsel, strip, tws, trank, bar_id, lane, nullptr, cstg,
+                col_item<N, PREC, N, false, CSTG>(P, lo + i, hsel, strip, tws, trank, bar_id, lane, nullptr, cstg,
                                                  lo + i + GE::TEAMS < hi ? lo + i + GE::TEAMS : -1);
                 any = true;
             }

@@ -47,7 +47,7 @@ cudaError_t launch_col_t(const Params& P, int hsel, int grid, cudaStream_t st) {
 
 template <bool PREC, bool HEAT, bool TS = false>
 cudaError_t launch_persist_t(const Params& P, int grid, cudaStream_t st) {
-    const int smem = TS ? GE::CTA_SMEM_TAB : GE::CTA_SMEM;
+    const int smem = TS ? GE::CTA_SMEM_TAB : GE::CTA_SMEM + ((!HEAT && GE::STAGE_COL) ? GE::COL_STAGE_SMEM : 0);
     cudaError_t e = set_smem(k_persist<N, PREC, HEAT, TS>, smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
