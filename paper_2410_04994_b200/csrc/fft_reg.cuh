@@ -129,6 +129,74 @@ __device__ __forceinline__ void dif_stages(float2 (&v)[R]) {
     }
 }
 
+// ---- radix-2^2 arrangement of the same butterflies -------------------------------------------------------------
+// The decimation-in-frequency network above multiplies by W_{2 SPAN}^k after EVERY stage (32 points: 20 general
+// and 14 eighth-root twiddles).  Moving the twiddles of two consecutive stages behind the second one (He &
+// Torkelson's radix-2^2: the first stage of a pair keeps only the factor -i on the upper half of its differences,
+// the second stage none, then the outputs of the length-4S block are multiplied by W_{4S}^{k j}, j = 0, 2, 1, 3 for its
+// four quarters) leaves the butterfly topology and the bit-reversed output order unchanged and needs 16 general + 12
+// eighth-root twiddles per 32 points (16 points: 4 + 4 instead of 4 + 6).  The transforms run at the fp32 pipe's
+// throughput (tests/probes/fft_issue_rate.cu), so the saved operations are saved time.
+
+// d * W_32^E (fwd; conj for INV) for E = 0..31: E >= 16 is the negative of E - 16 (folded into the constants)
+template <int E, bool INV, bool PREC>
+__device__ __forceinline__ float2 twmul32x(float2 d) {
+    if constexpr (E < 16) {
+        return twmul32<E, INV, PREC>(d);
+    } else if constexpr ((E - 16) % 4 == 0) {
+        const float2 r = twmul32<E - 16, INV, PREC>(d);
+        return make_float2(-r.x, -r.y);
+    } else {
+        constexpr float Wr = hi_of(-cos32(E - 16)), wr = lo_of(-cos32(E - 16));
+        constexpr float Wi = hi_of(sin32(E - 16)), wi = lo_of(sin32(E - 16));
+        return cmul_hl<INV, PREC>(d, Wr, Wi, wr, wi);
+    }
+}
+
+// (a, b) -> a + b and (a - b) * W_32^E
+template <int R, int I0, int I1, int E, bool INV, bool PREC>
+__device__ __forceinline__ void bfly_tw(float2 (&v)[R]) {
+    const float2 a = v[I0], b = v[I1];
+    v[I0] = __fadd2_rn(a, b);
+    if constexpr (E % 16 == 8) v[I1] = twmul32x<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));   // (+-i: scalar, see dif_bfly)
+    else v[I1] = twmul32x<E, INV, PREC>(__fadd2_rn(a, make_float2(-b.x, -b.y)));
+}
+// (a, b) -> (a + b) * W_32^E0 and (a - b) * W_32^E1
+template <int R, int I0, int I1, int E0, int E1, bool INV, bool PREC>
+__device__ __forceinline__ void bfly_tw2(float2 (&v)[R]) {
+    const float2 a = v[I0], b = v[I1];
+    v[I0] = twmul32x<E0, INV, PREC>(__fadd2_rn(a, b));
+    if constexpr (E1 % 16 == 8) v[I1] = twmul32x<E1, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));
+    else v[I1] = twmul32x<E1, INV, PREC>(__fadd2_rn(a, make_float2(-b.x, -b.y)));
+}
+
+template <int R, int BASE, int LEN, bool INV, bool PREC, int... K>
+__device__ __forceinline__ void r22_stage_a(float2 (&v)[R], std::integer_sequence<int, K...>) {
+    constexpr int S = LEN / 4;
+    (bfly_tw<R, BASE + K, BASE + K + 2 * S, (K >= S ? 8 : 0), INV, PREC>(v), ...);        // K = 0 .. 2S-1
+}
+template <int R, int BASE, int LEN, bool INV, bool PREC, int... K>
+__device__ __forceinline__ void r22_stage_b(float2 (&v)[R], std::integer_sequence<int, K...>) {
+    constexpr int S = LEN / 4, U = 32 / LEN;                                              // W_LEN = W_32^U
+    (bfly_tw<R, BASE + K, BASE + K + S, 2 * K * U, INV, PREC>(v), ...);                   // quarters j = 0, 2
+    (bfly_tw2<R, BASE + 2 * S + K, BASE + 3 * S + K, K * U, 3 * K * U, INV, PREC>(v), ...);   // quarters j = 1, 3
+}
+
+template <int R, int BASE, int LEN, bool INV, bool PREC>
+__device__ __forceinline__ void r22(float2 (&v)[R]) {
+    if constexpr (LEN == 2) {
+        bfly_tw<R, BASE, BASE + 1, 0, INV, PREC>(v);
+    } else if constexpr (LEN >= 4) {
+        constexpr int S = LEN / 4;
+        r22_stage_a<R, BASE, LEN, INV, PREC>(v, std::make_integer_sequence<int, 2 * S>{});
+        r22_stage_b<R, BASE, LEN, INV, PREC>(v, std::make_integer_sequence<int, S>{});
+        r22<R, BASE, S, INV, PREC>(v);
+        r22<R, BASE + S, S, INV, PREC>(v);
+        r22<R, BASE + 2 * S, S, INV, PREC>(v);
+        r22<R, BASE + 3 * S, S, INV, PREC>(v);
+    }
+}
+
 __host__ __device__ constexpr int bitrev(int i, int n) {
     int r = 0;
     for (int b = 1; b < n; b <<= 1) { r = (r << 1) | (i & 1); i >>= 1; }
@@ -151,7 +219,11 @@ __device__ __forceinline__ void brev_all(float2 (&v)[R], std::integer_sequence<i
 template <int R, bool INV, bool PREC>
 __device__ __forceinline__ void fft_reg(float2 (&v)[R]) {
     static_assert(R == 2 || R == 4 || R == 8 || R == 16 || R == 32, "radix");
+#ifdef SHG_FFT_RADIX2
     dif_stages<R, R / 2, INV, PREC>(v);
+#else
+    r22<R, 0, R, INV, PREC>(v);
+#endif
     brev_all<R>(v, std::make_integer_sequence<int, R>{});
 }
 

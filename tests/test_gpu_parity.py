@@ -79,8 +79,10 @@ def check(w, g1, g2, gh, o1, o2, oh, members=None, tol_field=TOL_FIELD, tol_eta=
         eta_g = hg[-1, 1] / (hg[0, 0] + hg[0, 1])
         eta_o = ho[-1, 1] / (ho[0, 0] + ho[0, 1])
         assert abs(eta_g / eta_o - 1) <= tol_eta, "eta member %d: %.8g vs %.8g" % (b, eta_g, eta_o)
-        # whole history: FH relative to itself, SH relative to the input power (SH starts at 0)
-        p0 = ho[0, 0] + ho[0, 1]
+        # whole history relative to the power scale of the run: the input power (SH starts at 0) -- or, where a
+        # deliberately unstable RK4 step amplifies the fields (nz = 1 at kW powers gains 13x in the oracle too,
+        # DESIGN.md 5.8), the largest power of the oracle's history
+        p0 = max(ho[0, 0] + ho[0, 1], float(np.max(ho)))
         assert np.max(np.abs(hg[:, 0] - ho[:, 0])) / p0 <= tol_eta
         assert np.max(np.abs(hg[:, 1] - ho[:, 1])) / p0 <= tol_eta
 
@@ -459,7 +461,10 @@ def test_record_every_thins_the_history_without_changing_it(name, nz, every, clu
 def test_linear_path_has_no_power_drift_over_many_steps():
     """Free propagation (d_eff = 0, no absorption) over 2000 steps with a per-step diffraction angle of ~1e-4
     rad: the power must stay put.  Guards the operand order of cmul_hl (fft_reg.cuh): with the product by
-    W.re in an inner fma the run gains 7e-9 of power per step (1.4e-5 here, 3e-4 of SH efficiency on cfg5)."""
+    W.re in an inner fma the run gains 7e-9 of power per step (1.4e-5 here, 3e-4 of SH efficiency on cfg5).
+    Correct code wanders by 0.4e-6 .. 4e-6 over these 2000 steps depending on the line length and on the order of
+    the butterflies (deterministic rounding patterns, no trend: DESIGN.md 5.1 has the table); the bound sits
+    between that and the bias it guards against."""
     c = wl.crystal(40e-3, d_eff=0.0)
     bm = wl.beam(c, 100.0, 2.84, 10.0)
     n, nz = 256, 2000
@@ -469,7 +474,7 @@ def test_linear_path_has_no_power_drift_over_many_steps():
     ctx.propagate(torch.from_numpy(wl.gaussian_pump(n, n, c, bm)[None]).cuda())
     torch.cuda.synchronize()
     h = ctx.power_history(0)
-    assert np.max(np.abs(h[:, 0] / h[0, 0] - 1)) <= 2e-6
+    assert np.max(np.abs(h[:, 0] / h[0, 0] - 1)) <= 5e-6
 
 
 # ------------------------------------------------------------------------------------------------
