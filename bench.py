@@ -249,10 +249,12 @@ def workload_label(w):
 # B200 arm
 # ------------------------------------------------------------------------------------------------
 def kernel_label(ctx, g, per_pass):
-    if ctx.last_cluster_size():
+    k = ctx.last_kernel()
+    if k == 4:
         return "k_cluster<%d,%d>" % (g["nx"], ctx.last_cluster_size())
-    if not per_pass and g["nx"] == g["ny"]:
-        return "k_persist<%d>" % g["nx"]
+    names = {1: "k_persist", 2: "k_persist_flat", 3: "k_persist_pipe", 5: "k_persist_paper"}
+    if k in names:
+        return "%s<%d>" % (names[k], g["nx"])
     return "k_row+k_col"
 
 

@@ -222,6 +222,11 @@ int shg_last_launch_count(const shg_ctx* ctx);
 /* Cluster size (8 or 16) when the last propagate ran in the cluster kernel (SHG_OPT_CLUSTER), else 0. */
 int shg_last_cluster_size(const shg_ctx* ctx);
 
+/* Which kernel ran the z-loop of the last propagate: 0 = two launches per z-step (k_row + k_col), 1 = k_persist,
+ * 2 = k_persist_flat (sparse launch), 3 = k_persist_pipe (SHG_OPT_PIPELINE), 4 = k_cluster, 5 = k_persist_paper
+ * (SHG_OPT_SCHEME = 1).  Lets bench.py and the tests name what they measured. */
+int shg_last_kernel(const shg_ctx* ctx);
+
 void shg_destroy(shg_ctx* ctx);
 
 const char* shg_strerror(int code);

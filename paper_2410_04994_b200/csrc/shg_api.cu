@@ -242,6 +242,7 @@ struct shg_ctx {
     int last_batch = 0;
     int last_launches = 0;
     int last_cluster = 0;               // cluster size of the last propagate (0: batched kernels)
+    int last_kernel = 0;                // shg_last_kernel
     bool hist_valid = false;
     int last_scheme = 0;
     std::vector<double> hist_host;       // [batch][nrec+1][2], W
@@ -695,6 +696,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
                 ctx->last_launches = launches;
                 ctx->last_scheme = 0;
                 ctx->last_cluster = csize;
+                ctx->last_kernel = 4;
                 ctx->hist_valid = false;
                 return SHG_OK;
             }
@@ -747,7 +749,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
         const int ipc = (UR + grid_p - 1) / grid_p;
         const int warps_per_slot = ix.warps / ix.row_slots;
-        P.flat_rows = (use_persist && ctx->scheme == 0 && !P.Q && ipc <= ix.row_slots &&
+        P.flat_rows = (use_persist && !P.pipeline && ctx->scheme == 0 && !P.Q && ipc <= ix.row_slots &&
                        2 * ipc * warps_per_slot <= ix.warps) ? 1 : 0;
     }
 
@@ -760,11 +762,12 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
         if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
         bool looped = false;
+        ctx->last_kernel = 0;
         if (use_persist && g.nz > 1) {
             const int grid_p = grid_r > grid_c ? grid_r : grid_c;
             ctx->trace_grid = grid_p;
             const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
-            if (e == cudaSuccess) { ++launches; looped = true; }
+            if (e == cudaSuccess) { ++launches; looped = true; ctx->last_kernel = 5; }
             else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
         }
         if (!looped) {
@@ -781,11 +784,12 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     CU(ctx->Ly.col(P, 1, prec, grid_c, st)); ++launches;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
     bool looped = false;
+    ctx->last_kernel = 0;
     if (use_persist) {
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
         ctx->trace_grid = grid_p;
         const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
-        if (e == cudaSuccess) { ++launches; looped = true; }
+        if (e == cudaSuccess) { ++launches; looped = true; ctx->last_kernel = P.flat_rows ? 2 : (P.pipeline ? 3 : 1); }
         else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
     }
     if (!looped) {
@@ -991,5 +995,6 @@ static int measure_fp32(double* tflops, bool distinct) {
 int shg_last_launch_count(const shg_ctx* ctx) { return ctx ? ctx->last_launches : SHG_EINVAL; }
 
 int shg_last_cluster_size(const shg_ctx* ctx) { return ctx ? ctx->last_cluster : SHG_EINVAL; }
+int shg_last_kernel(const shg_ctx* ctx) { return ctx ? ctx->last_kernel : SHG_EINVAL; }
 
 }  // extern "C"

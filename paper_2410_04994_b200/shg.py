@@ -22,7 +22,7 @@ EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_tempe
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
            "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
            "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
-           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct")
+           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct", "shg_last_kernel")
 
 
 class Grid(C.Structure):
@@ -75,6 +75,7 @@ def lib():
     L.shg_read_trace.argtypes = [vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.shg_last_launch_count.argtypes = [vp]
     L.shg_last_cluster_size.argtypes = [vp]
+    L.shg_last_kernel.argtypes = [vp]
     L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
     L.shg_measure_fp32_peak.argtypes = [dp]
     L.shg_measure_fp32_peak_distinct.argtypes = [dp]
@@ -304,6 +305,10 @@ class Shg:
 
     def last_cluster_size(self) -> int:
         return int(lib().shg_last_cluster_size(self._h))
+
+    def last_kernel(self) -> int:
+        """0 k_row + k_col, 1 k_persist, 2 k_persist_flat, 3 k_persist_pipe, 4 k_cluster, 5 k_persist_paper."""
+        return int(lib().shg_last_kernel(self._h))
 
     def close(self):
         if getattr(self, "_h", None):

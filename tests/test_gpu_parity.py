@@ -320,11 +320,11 @@ def test_pipelined_batched_kernel_gives_the_same_bits(n, B, nz, nzt):
              per_member=bool(nzt), A1=A1)
     base = {shg.OPT_CLUSTER: 0, shg.OPT_PIPELINE: 2}
     p1, p2, ph, cp = run_gpu(w, A2=A2, options=base)
-    assert cp.last_launch_count() == 5
+    assert cp.last_launch_count() == 5 and cp.last_kernel() == 3          # k_persist_pipe
     q1, q2, qh, cq = run_gpu(w, A2=A2, options={shg.OPT_CLUSTER: 0, shg.OPT_PIPELINE: 0})
-    assert cq.last_launch_count() == 5
+    assert cq.last_launch_count() == 5 and cq.last_kernel() in (1, 2)     # k_persist / k_persist_flat
     r1, r2, rh, cr = run_gpu(w, A2=A2, options=base, persistent=False)
-    assert cr.last_launch_count() == 4 + 2 * nz
+    assert cr.last_launch_count() == 4 + 2 * nz and cr.last_kernel() == 0
     for a1, a2, ah in ((q1, q2, qh), (r1, r2, rh)):
         assert np.array_equal(p1, a1) and np.array_equal(p2, a2)
         assert all(np.array_equal(ph[b], ah[b]) for b in range(B))
