@@ -335,6 +335,21 @@ def test_pipelined_batched_kernel_gives_the_same_bits(n, B, nz, nzt):
     assert np.array_equal(s1.cpu().numpy(), p1) and np.array_equal(s2.cpu().numpy(), p2)
 
 
+@pytest.mark.parametrize("name,batch,nz,mode", [("stream256", 48, 60, 1), ("stream1024", 4, 30, 2), ("cfg4", 64, 40, 2)])
+def test_pipelined_kernel_at_scale_gives_the_same_bits(name, batch, nz, mode):
+    """The pipelined batched kernel with every SM busy for many z-steps (where a missing dependency between its
+    split-phase barriers, its continuing round-robin deal or its staged strips would show) against k_persist:
+    identical fields and history for every member.  mode 1 = the library's own choice must be the pipelined kernel."""
+    w = wl.make(name, nz=nz, batch=batch)
+    p1, p2, ph, cp = run_gpu(w, options={shg.OPT_PIPELINE: mode})
+    assert cp.last_kernel() == 3
+    q1, q2, qh, cq = run_gpu(w, options={shg.OPT_PIPELINE: 0})
+    assert cq.last_kernel() == 1
+    assert np.array_equal(p1, q1) and np.array_equal(p2, q2)
+    assert all(np.array_equal(ph[b], qh[b]) for b in range(batch))
+    assert np.isfinite(p1).all() and min(h[-1, 1] for h in ph) > 0
+
+
 def test_free_diffraction_matches_analytic_beam_on_gpu():
     """d_eff = 0: the GPU linear path alone against Eq. 5, no oracle involved."""
     n = 256
