@@ -142,8 +142,13 @@ int shg_set_option(shg_ctx* ctx, int option, int value);
  * and must stay valid and unchanged until every propagate that uses it has completed. */
 int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, int per_member);
 
-/* Same, from a HOST array: copied (asynchronously on `cuda_stream` when the memory is pinned) into a
- * library-owned device buffer that is allocated on first use and reused afterwards. */
+/* Same, from a HOST array: copied (asynchronously when the memory is pinned) into a library-owned device buffer that is
+ * allocated on first use and reused afterwards.  A small array is copied on `cuda_stream` right away.  One array
+ * shared by all members of 32 MB or more is uploaded by the NEXT shg_propagate[_host] instead, in chunks of planes on
+ * the library's own copy stream, behind that call's field uploads: the persistent kernel of a single simulation is
+ * launched once per chunk, over the z-steps whose planes the chunk completes (a z-step reads only the planes around
+ * its two nodes), so the transfer of chunk c + 1 runs under the z-steps of chunk c; every other kernel waits for the
+ * last chunk.  T_host must therefore stay valid and unchanged until that propagate has completed. */
 int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform, int per_member,
                              void* cuda_stream);
 

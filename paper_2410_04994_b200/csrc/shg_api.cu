@@ -233,6 +233,15 @@ struct shg_ctx {
     double T_uniform = 0.0;
     int T_per_member = 0;
     bool T_set = false;
+    // A host temperature array is uploaded in chunks of planes on the library's own copy stream, one event per chunk,
+    // so that the persistent kernel can start on the first planes while the rest is still on its way
+    // (shg_set_temperature_host / shg_propagate).  up_chunks == 0: nothing pending, d_T is complete.
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t guard_ev = nullptr;
+    std::vector<cudaEvent_t> up_ev;
+    int up_chunks = 0, up_planes = 0;    // chunks of the current upload, planes per chunk
+    const float* up_host = nullptr;      // deferred upload: the host array that the next propagate copies, chunk by chunk,
+                                         // AFTER its own field uploads (the copy engine serves its queue in order)
 
     bool timing = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
@@ -394,6 +403,9 @@ void free_ctx(shg_ctx* ctx) {
     cudaFree(ctx->d_trace);
     for (int i = 0; i < 2; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    for (cudaEvent_t e : ctx->up_ev) cudaEventDestroy(e);
+    if (ctx->guard_ev) cudaEventDestroy(ctx->guard_ev);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     delete ctx;
 }
 
@@ -551,6 +563,7 @@ int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, i
     ctx->T_per_member = per_member ? 1 : 0;
     if (ctx->T_uniform != T_uniform) { ctx->T_uniform = T_uniform; ctx->tables_dirty = true; }
     ctx->T_set = true;
+    if (T_device != ctx->d_T_owned) { ctx->up_chunks = 0; ctx->up_host = nullptr; }
     return SHG_OK;
 }
 
@@ -567,6 +580,20 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
         ctx->T_owned_bytes = 0;
         CU(cudaMalloc((void**)&ctx->d_T_owned, bytes));
         ctx->T_owned_bytes = bytes;
+    }
+    // One array for all members, large enough to matter: upload it plane chunk by plane chunk on the copy stream
+    // (after whatever the caller's stream and the last propagate still have in flight), one event per chunk.
+    // shg_propagate makes its kernels wait for the chunks they need: the persistent kernel of a single simulation
+    // runs the z-steps that the first chunk covers while the second is copied, and so on (a z-step reads the planes
+    // around its two nodes only, G15), everything else waits for the last chunk.
+    const int nzt = ctx->g.nzt;
+    ctx->up_chunks = 0;
+    ctx->up_host = nullptr;
+    if (!(per_member && ctx->g.batch > 1) && nzt >= 8 && bytes >= ((size_t)32 << 20)) {
+        // deferred: the next shg_propagate enqueues the chunked copy (enqueue_upload) behind its own field uploads
+        const int rc = shg_set_temperature(ctx, ctx->d_T_owned, T_uniform, per_member);
+        ctx->up_host = T_host;
+        return rc;
     }
     CU(cudaMemcpyAsync(ctx->d_T_owned, T_host, bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
     return shg_set_temperature(ctx, ctx->d_T_owned, T_uniform, per_member);
@@ -590,6 +617,43 @@ int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq) {
     }
     ctx->d_Q = Q_device;
     ctx->nq = nq;
+    return SHG_OK;
+}
+
+// The chunked upload of a host temperature array that shg_set_temperature_host deferred: plane chunk by plane chunk
+// on the library's copy stream, after everything the propagate's stream (its field uploads) and the last propagate
+// have in flight, one event per chunk.
+static int enqueue_upload(shg_ctx* ctx, cudaStream_t st) {
+    const float* T_host = ctx->up_host;
+    ctx->up_host = nullptr;
+    const int nzt = ctx->g.nzt;
+    const size_t plane_f = np_of(ctx);
+    const size_t bytes = sizeof(float) * (size_t)nzt * plane_f;
+    if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    if (!ctx->guard_ev) CU(cudaEventCreateWithFlags(&ctx->guard_ev, cudaEventDisableTiming));
+    int chunks = (int)(bytes >> 26);                           // ~64 MB each
+    chunks = chunks < 2 ? 2 : (chunks > 16 ? 16 : chunks);
+    const int planes = (nzt + chunks - 1) / chunks;
+    chunks = (nzt + planes - 1) / planes;
+    while ((int)ctx->up_ev.size() < chunks) {
+        cudaEvent_t e;
+        CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->up_ev.push_back(e);
+    }
+    CU(cudaEventRecord(ctx->guard_ev, st));
+    CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->guard_ev, 0));
+    if (ctx->last_stream != st && ctx->last_batch != 0) {      // the last propagate (another stream) may still read T
+        CU(cudaEventRecord(ctx->guard_ev, ctx->last_stream));
+        CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->guard_ev, 0));
+    }
+    for (int c = 0; c < chunks; ++c) {
+        const int p0 = c * planes, p1 = (p0 + planes < nzt) ? p0 + planes : nzt;
+        CU(cudaMemcpyAsync(ctx->d_T_owned + (size_t)p0 * plane_f, T_host + (size_t)p0 * plane_f,
+                           sizeof(float) * (size_t)(p1 - p0) * plane_f, cudaMemcpyHostToDevice, ctx->copy_stream));
+        CU(cudaEventRecord(ctx->up_ev[(size_t)c], ctx->copy_stream));
+    }
+    ctx->up_chunks = chunks;
+    ctx->up_planes = planes;
     return SHG_OK;
 }
 
@@ -630,6 +694,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     const shg_grid& g = ctx->g;
     shg::Params P{};
     P.nx = g.nx; P.ny = g.ny; P.nz = g.nz; P.nzt = g.nzt; P.batch = batch;
+    P.n_begin = 0; P.n_end = g.nz;
     P.ny_log2 = 0;
     while ((1 << P.ny_log2) < g.ny) ++P.ny_log2;
     P.A[0] = (float2*)A1_out; P.A[1] = (float2*)A2_out;
@@ -653,6 +718,25 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
 
     const size_t np = np_of(ctx);
     int launches = 0;
+    // A host temperature array may still be on its way (shg_set_temperature_host): kernels that read T wait for the
+    // chunk events.  pending: this propagate reads the library's copy and an upload is outstanding.
+    if (ctx->up_host != nullptr && P.T != nullptr && P.T == ctx->d_T_owned) {
+        const int rc = enqueue_upload(ctx, st);
+        if (rc != SHG_OK) return rc;
+    }
+    const bool pending = ctx->up_chunks > 0 && P.T != nullptr && P.T == ctx->d_T_owned;
+    auto wait_all_chunks = [&]() -> cudaError_t {
+        return pending ? cudaStreamWaitEvent(st, ctx->up_ev[(size_t)ctx->up_chunks - 1], 0) : cudaSuccess;
+    };
+    // highest temperature plane that z-step n reads: the planes around its two nodes n and n + 1 (G15, t_node)
+    auto last_plane_of_step = [&](int n) {
+        if (g.nzt <= 1) return 0;
+        const long long num = (long long)(n + 1) * (g.nzt - 1);
+        long long k = num / g.nz;
+        long long rem = num - k * g.nz;
+        if (k > g.nzt - 2) { k = g.nzt - 2; rem = g.nz; }
+        return (int)(k + (rem != 0 ? 1 : 0));
+    };
     CU(cudaMemsetAsync(ctx->d_hfix, 0, sizeof(long long) * (size_t)g.batch * (ctx->nrec + 1) * 2, st));
     CU(cudaMemsetAsync(ctx->d_barrier, 0, 8 * sizeof(unsigned int), st));
     if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
@@ -686,6 +770,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         if (csize != 0) {
             P.trace_grid = batch * csize < ctx->sm_count ? batch * csize : ctx->sm_count;
             ctx->trace_grid = P.trace_grid;
+            CU(wait_all_chunks());
             if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
             const cudaError_t e = ctx->Lx.cluster(P, csize, true, nullptr, st);
             if (e == cudaSuccess) {
@@ -697,6 +782,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
                 ctx->last_scheme = 0;
                 ctx->last_cluster = csize;
                 ctx->last_kernel = 4;
+                if (pending) ctx->up_chunks = 0;
                 ctx->hist_valid = false;
                 return SHG_OK;
             }
@@ -758,6 +844,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         // half-step of step 0, the row pass n of the loop the second half of step n and the first half of step
         // n + 1, ROW_FINAL the second half of step nz - 1; every linear step is a full dz (tables 0).
         if (!prec || P.Q) return SHG_EINVAL;     // this variant: hi+lo constants only, no heat output
+        CU(wait_all_chunks());
         CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 0, prec, grid_r, st)); ++launches;
         CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
         if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], st));
@@ -788,11 +875,39 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     if (use_persist) {
         const int grid_p = grid_r > grid_c ? grid_r : grid_c;
         ctx->trace_grid = grid_p;
-        const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
-        if (e == cudaSuccess) { ++launches; looped = true; ctx->last_kernel = P.flat_rows ? 2 : (P.pipeline ? 3 : 1); }
-        else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
+        if (pending && !P.pipeline) {
+            // Temperature array still uploading: one launch per chunk, over the z-steps whose planes that chunk
+            // completes (k_persist / k_persist_flat take a step range; the device-wide barrier counts from zero in
+            // every launch).  The copy of chunk c + 1 runs under the z-steps of chunk c.
+            int n0 = 0;
+            for (int c = 0; c < ctx->up_chunks && n0 < g.nz; ++c) {
+                const int have = (c + 1) * ctx->up_planes < g.nzt ? (c + 1) * ctx->up_planes : g.nzt;   // planes [0, have)
+                int n1 = n0;
+                while (n1 < g.nz && last_plane_of_step(n1) < have) ++n1;
+                if (c == ctx->up_chunks - 1) n1 = g.nz;
+                if (n1 == n0) continue;
+                CU(cudaStreamWaitEvent(st, ctx->up_ev[(size_t)c], 0));
+                if (n0 > 0) CU(cudaMemsetAsync(ctx->d_barrier, 0, sizeof(unsigned int), st));
+                P.n_begin = n0; P.n_end = n1;
+                const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
+                if (e != cudaSuccess) {
+                    if (n0 == 0 && coop_unavailable(e)) break;             // fall back to the per-pass launches below
+                    return cuda_fail(e, "persistent kernel launch");
+                }
+                ++launches; looped = true;
+                n0 = n1;
+            }
+            P.n_begin = 0; P.n_end = g.nz;
+            if (looped) ctx->last_kernel = P.flat_rows ? 2 : 1;
+        } else {
+            CU(wait_all_chunks());
+            const cudaError_t e = ctx->Lx.persist(P, prec, grid_p, st);
+            if (e == cudaSuccess) { ++launches; looped = true; ctx->last_kernel = P.flat_rows ? 2 : (P.pipeline ? 3 : 1); }
+            else if (!coop_unavailable(e)) return cuda_fail(e, "persistent kernel launch");
+        }
     }
     if (!looped) {
+        CU(wait_all_chunks());
         for (int n = 0; n < g.nz; ++n) {
             const int hsel = (n == g.nz - 1) ? 1 : 0;
             CU(ctx->Lx.row(P, shg::ROW_MID, n, hsel, prec, grid_r, st)); ++launches;
@@ -808,6 +923,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
     ctx->last_launches = launches;
     ctx->last_scheme = ctx->scheme;
     ctx->hist_valid = false;
+    if (pending) ctx->up_chunks = 0;         // this stream has waited for every chunk: the copy is complete for what follows
     return SHG_OK;
 }
 

@@ -1209,7 +1209,7 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         epoch += 1;
         const unsigned int target = epoch * gridDim.x;
         asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(P.barrier), "r"(1u) : "memory");
-        if (sc_next != nullptr && n + 1 < P.nz) ctx_step(P, *sc_next, n + 1);
+        if (sc_next != nullptr && n + 1 < P.n_end) ctx_step(P, *sc_next, n + 1);
         int good = 1;
         if (ld_relaxed_u32(P.barrier) < target) {
             const long long t0 = clock64();
@@ -1275,15 +1275,15 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist(Params P) {
     __shared__ unsigned long long s_pow[2];
     __shared__ StepCtx sc;
     if (threadIdx.x < 2) s_pow[threadIdx.x] = 0ull;
-    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, 0); }
+    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, P.n_begin); }
     unsigned long long* sp = (P.batch == 1) ? s_pow : nullptr;
     __syncthreads();
-    stage_tables(P.nz == 1 ? 1 : 0);
+    stage_tables(P.n_begin == P.nz - 1 ? 1 : 0);
     unsigned int epoch = 0;
 #pragma unroll 1
-    for (int n = 0; n < P.nz; ++n) {
+    for (int n = P.n_begin; n < P.n_end; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
-        if (hsel == 1 && n > 0) stage_tables(1);             // (every warp passed the barrier's closing bar.sync)
+        if (hsel == 1 && n > P.n_begin) stage_tables(1);     // (every warp passed the barrier's closing bar.sync)
         row_pass<N, ROW_MID, PREC, HEAT, TS>(P, sc, n, hsel, smem_cta, tws, warp, lane, stab, sp);
         if (sp) flush_powers(P, sc, sp);
         if (!grid_barrier(P, epoch, n, 0)) return;
@@ -1302,12 +1302,12 @@ __global__ void __launch_bounds__(Geo<N>::THREADS, 1) k_persist_flat(Params P) {
     __shared__ unsigned long long s_acc[2 * Geo<N>::ROW_SLOTS * Geo<N>::HG];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     __shared__ StepCtx sc;
-    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, 0); }
+    if (threadIdx.x == 32) { ctx_rows<N>(P, sc); ctx_cols<N>(P, sc); ctx_step(P, sc, P.n_begin); }
     const float4* tws = load_twiddles<N>(smem_raw, P.twx);
     float2* smem_cta = reinterpret_cast<float2*>(smem_raw);
     unsigned int epoch = 0;
 #pragma unroll 1
-    for (int n = 0; n < P.nz; ++n) {
+    for (int n = P.n_begin; n < P.n_end; ++n) {
         const int hsel = (n == P.nz - 1) ? 1 : 0;
         row_pass_flat<N, PREC>(P, sc, n, hsel, smem_cta, tws, warp, lane, s_acc);
         if (!grid_barrier(P, epoch, n, 0)) return;

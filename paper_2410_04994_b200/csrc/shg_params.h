@@ -21,6 +21,8 @@ struct MemberDev {
 
 struct Params {
     int nx, ny, nz, nzt, batch;
+    int n_begin, n_end;        // z-steps [n_begin, n_end) of this launch of a persistent kernel (normally 0, nz; a host
+                               // temperature array that is still being uploaded is consumed range by range, shg_api.cu)
     int ny_log2;               // ny = 1 << ny_log2 (every supported line length is a power of two)
     int flat_rows;             // 1: sparse launch, the persistent kernel spreads the nonlinear step over the CTA (row_pass_flat)
     int scheme;                // 0: L/2 - N - L/2 with merged half-steps; 1: the paper's N/2 - L - N/2 (SHG_OPT_SCHEME)

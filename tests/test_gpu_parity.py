@@ -392,6 +392,33 @@ def test_gaussian_input_kernel_and_host_buffer_path():
     assert rel_l2(n1.cpu().numpy(), g1) < 1e-5
 
 
+@pytest.mark.parametrize("name,nz", [("cfg5", 600), ("cfg3", 300), ("cfg5", 3)])
+def test_overlapped_temperature_upload_gives_the_same_bits(name, nz):
+    """shg_set_temperature_host uploads a large temperature array in chunks of planes on the library's copy stream
+    and shg_propagate launches the persistent kernel once per chunk, over the z-steps whose planes that chunk
+    completes (k_persist for cfg5's 1 GiB array of 256 planes, k_persist_flat for cfg3's planes on the nodes): same
+    fields and history as with the whole array resident on the device before the launch, also when the same context
+    propagates again without a new upload, and from pageable as well as pinned host memory."""
+    w = wl.make(name, nz=nz)
+    g1, g2, gh, cg = run_gpu(w)                                       # device-resident T: one launch of the z-loop
+    assert cg.last_launch_count() == 5
+    ctx = shg.Shg(w["grid"], w["crystal"], w["beams"])
+    Tpin = torch.from_numpy(w["T"]).pin_memory()
+    for T in (Tpin, w["T"]):
+        ctx.set_temperature(T)                                        # host array -> chunked upload
+        A1 = torch.from_numpy(w["A1"]).cuda()
+        h1, h2 = ctx.propagate(A1)
+        ctx.synchronize()
+        assert ctx.last_launch_count() > 5 or nz < 40                 # several ranges (a 3-step run needs one chunk)
+        assert np.array_equal(h1.cpu().numpy(), g1) and np.array_equal(h2.cpu().numpy(), g2)
+        assert np.array_equal(ctx.power_history(0), gh[0])
+    r1, r2 = ctx.propagate(A1)                                        # again, nothing pending: one launch
+    ctx.synchronize()
+    assert ctx.last_launch_count() == 5
+    assert np.array_equal(r1.cpu().numpy(), g1) and np.array_equal(r2.cpu().numpy(), g2)
+    ctx.close()
+
+
 def test_precise_constants_matter_over_many_steps():
     """with plain fp32 constants the error grows linearly with the step count; the hi+lo
     constants keep cfg2 (1000 steps) well inside the tolerance."""
