@@ -324,7 +324,7 @@ __device__ __forceinline__ void nl_rhs(float2 a1, float2 a2, const PhaseCoef& pc
     float px = fmaf(a2.x, a1.x, a2.y * a1.y);            // A2 conj(A1)
     float py = fmaf(a2.y, a1.x, -a2.x * a1.y);
     float qx = fmaf(a1.x, a1.x, -a1.y * a1.y);           // A1^2
-    float qy = 2.0f * a1.x * a1.y;
+    float qy = (2.0f * a1.x) * a1.y;
     d1.x = fmaf(px, pc.u1x, -py * pc.u1y);
     d1.y = fmaf(px, pc.u1y, py * pc.u1x);
     d2.x = fmaf(qx, pc.u2x, -qy * pc.u2y);
@@ -352,11 +352,73 @@ __device__ __forceinline__ void rk4_point(float2& a1, float2& a2, const PhaseCoe
            make_float2(fmaf(0.5f, k2b.x, a2.x), fmaf(0.5f, k2b.y, a2.y)), cm, g1, g2, k3a, k3b);
     nl_rhs(make_float2(a1.x + k3a.x, a1.y + k3a.y), make_float2(a2.x + k3b.x, a2.y + k3b.y), cb, g1, g2,
            k4a, k4b);
+    // a += (k1 + 2 (k2 + k3) + k4) / 6, every rounding spelled out (the packed twin rk4_point2 repeats them)
     constexpr float S = 1.0f / 6.0f;
-    a1.x += S * (k1a.x + 2.0f * (k2a.x + k3a.x) + k4a.x);
-    a1.y += S * (k1a.y + 2.0f * (k2a.y + k3a.y) + k4a.y);
-    a2.x += S * (k1b.x + 2.0f * (k2b.x + k3b.x) + k4b.x);
-    a2.y += S * (k1b.y + 2.0f * (k2b.y + k3b.y) + k4b.y);
+    a1.x = fmaf(S, fmaf(2.0f, k2a.x + k3a.x, k1a.x) + k4a.x, a1.x);
+    a1.y = fmaf(S, fmaf(2.0f, k2a.y + k3a.y, k1a.y) + k4a.y, a1.y);
+    a2.x = fmaf(S, fmaf(2.0f, k2b.x + k3b.x, k1b.x) + k4b.x, a2.x);
+    a2.y = fmaf(S, fmaf(2.0f, k2b.y + k3b.y, k1b.y) + k4b.y, a2.y);
+}
+
+// ---- the same for TWO points at once in Blackwell's packed fp32x2 instructions (FFMA2 / FMUL2 / FADD2) ----------
+// A float2 here is NOT a complex number but one real quantity of two points (.x = point q, .y = point q + 1).  The
+// nonlinear step is bound by instruction issue (232 instructions per point, 174 of them fp32 arithmetic, at 0.84 per
+// clock with four warps per scheduler: profiles/r02b_summary.md 3); a packed instruction does the arithmetic of both
+// points in one issue slot.  Every operation is the one of the scalar code above, in the same order, so both give
+// the same bits.  What made an earlier attempt useless (+186 MOVs to form the pairs) was the complex
+// (re, im) layout of the line in shared memory; row_item now writes the line "split" for the nonlinear step --
+// (re_q, re_q+1) and (im_q, im_q+1) as two 8-byte records -- so that the pairs arrive as pairs.
+struct PhaseCoef2 { float2 u1x, u1y, u2x, u2y; };
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 ng2(float2 a) { return make_float2(-a.x, -a.y); }
+
+__device__ __forceinline__ PhaseCoef2 phase_coef2(float2 c, float2 s, float k1, float k2) {
+    PhaseCoef2 pc;
+    pc.u1x = __fmul2_rn(bc2(k1), s); pc.u1y = __fmul2_rn(bc2(k1), c);
+    pc.u2x = __fmul2_rn(bc2(-k2), s); pc.u2y = __fmul2_rn(bc2(k2), c);
+    return pc;
+}
+__device__ __forceinline__ PhaseCoef2 phase_coef2(const PhaseCoef& p) {
+    PhaseCoef2 pc;
+    pc.u1x = bc2(p.u1x); pc.u1y = bc2(p.u1y); pc.u2x = bc2(p.u2x); pc.u2y = bc2(p.u2y);
+    return pc;
+}
+
+__device__ __forceinline__ void nl_rhs2(float2 a1x, float2 a1y, float2 a2x, float2 a2y, const PhaseCoef2& pc, float g1,
+                                        float g2, float2& d1x, float2& d1y, float2& d2x, float2& d2y) {
+    const float2 px = __ffma2_rn(a2x, a1x, __fmul2_rn(a2y, a1y));            // A2 conj(A1)
+    const float2 py = __ffma2_rn(a2y, a1x, __fmul2_rn(ng2(a2x), a1y));
+    const float2 qx = __ffma2_rn(a1x, a1x, __fmul2_rn(ng2(a1y), a1y));       // A1^2
+    const float2 qy = __fmul2_rn(__fmul2_rn(bc2(2.0f), a1x), a1y);
+    d1x = __ffma2_rn(px, pc.u1x, __fmul2_rn(ng2(py), pc.u1y));
+    d1y = __ffma2_rn(px, pc.u1y, __fmul2_rn(py, pc.u1x));
+    d2x = __ffma2_rn(qx, pc.u2x, __fmul2_rn(ng2(qy), pc.u2y));
+    d2y = __ffma2_rn(qx, pc.u2y, __fmul2_rn(qy, pc.u2x));
+    if (g1 != 0.f) {
+        const float2 t1 = __fmul2_rn(bc2(-g1), __ffma2_rn(a1x, a1x, __fmul2_rn(a1y, a1y)));
+        d1x = __ffma2_rn(t1, a1x, d1x); d1y = __ffma2_rn(t1, a1y, d1y);
+    }
+    if (g2 != 0.f) {
+        const float2 t2 = __fmul2_rn(bc2(-g2), __ffma2_rn(a2x, a2x, __fmul2_rn(a2y, a2y)));
+        d2x = __ffma2_rn(t2, a2x, d2x); d2y = __ffma2_rn(t2, a2y, d2y);
+    }
+}
+
+__device__ __forceinline__ void rk4_point2(float2& a1x, float2& a1y, float2& a2x, float2& a2y, const PhaseCoef2& ca,
+                                           const PhaseCoef2& cm, const PhaseCoef2& cb, float g1, float g2) {
+    float2 k1ax, k1ay, k1bx, k1by, k2ax, k2ay, k2bx, k2by, k3ax, k3ay, k3bx, k3by, k4ax, k4ay, k4bx, k4by;
+    const float2 h = bc2(0.5f), two = bc2(2.0f), S = bc2(1.0f / 6.0f);
+    nl_rhs2(a1x, a1y, a2x, a2y, ca, g1, g2, k1ax, k1ay, k1bx, k1by);
+    nl_rhs2(__ffma2_rn(h, k1ax, a1x), __ffma2_rn(h, k1ay, a1y), __ffma2_rn(h, k1bx, a2x), __ffma2_rn(h, k1by, a2y), cm,
+            g1, g2, k2ax, k2ay, k2bx, k2by);
+    nl_rhs2(__ffma2_rn(h, k2ax, a1x), __ffma2_rn(h, k2ay, a1y), __ffma2_rn(h, k2bx, a2x), __ffma2_rn(h, k2by, a2y), cm,
+            g1, g2, k3ax, k3ay, k3bx, k3by);
+    nl_rhs2(__fadd2_rn(a1x, k3ax), __fadd2_rn(a1y, k3ay), __fadd2_rn(a2x, k3bx), __fadd2_rn(a2y, k3by), cb, g1, g2,
+            k4ax, k4ay, k4bx, k4by);
+    a1x = __ffma2_rn(S, __fadd2_rn(__ffma2_rn(two, __fadd2_rn(k2ax, k3ax), k1ax), k4ax), a1x);
+    a1y = __ffma2_rn(S, __fadd2_rn(__ffma2_rn(two, __fadd2_rn(k2ay, k3ay), k1ay), k4ay), a1y);
+    a2x = __ffma2_rn(S, __fadd2_rn(__ffma2_rn(two, __fadd2_rn(k2bx, k3bx), k1bx), k4bx), a2x);
+    a2y = __ffma2_rn(S, __fadd2_rn(__ffma2_rn(two, __fadd2_rn(k2by, k3by), k1by), k4by), a2y);
 }
 
 // Raw operands of one point's phase update: the (up to) two temperature planes around z_n and around
@@ -382,6 +444,22 @@ __device__ __forceinline__ float dT_lerp(float t0, float t1, float f, bool two, 
         a = fmaf(f, b - a, a);
     }
     return a;
+}
+
+__device__ __forceinline__ float2 dT_lerp2(float2 t0, float2 t1, float f, bool two, float Thi, float Tlo) {
+    float2 a = __fadd2_rn(__fadd2_rn(t0, bc2(-Thi)), bc2(-Tlo));
+    if (two) {
+        const float2 b = __fadd2_rn(__fadd2_rn(t1, bc2(-Thi)), bc2(-Tlo));
+        a = __ffma2_rn(bc2(f), __fadd2_rn(b, ng2(a)), a);
+    }
+    return a;
+}
+__device__ __forceinline__ float2 wrap_2pi2(float2 p) {
+    constexpr float TWO_PI_HI = 6.2831854820251465f, TWO_PI_LO = -1.7484555314695172e-07f;
+    const float2 t = __fmul2_rn(p, bc2(0.15915494309189535f));
+    const float2 k = make_float2(rintf(t.x), rintf(t.y));
+    p = __ffma2_rn(ng2(k), bc2(TWO_PI_HI), p);
+    return __ffma2_rn(ng2(k), bc2(TWO_PI_LO), p);
 }
 
 // Which T planes serve step node n: k = min(floor(n (nzt-1)/nz), nzt-2), f = frac.
@@ -518,9 +596,21 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             if constexpr (R >= 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
             nxt = t_load(Ta, Tn, plane, pbase + M, ta.two, tb.two, phi + M);
         }
-        // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2)
+        // conj(field), rotated for f = 1, goes to shared memory: register q <-> element M q + m (+ N/2).
+        // PK (no heat output): "split" image for the packed two-point RK4 -- slot M q + m holds (re_q, re_q+1) and
+        // slot M (q + 1) + m holds (im_q, im_q+1) for even q, instead of the complex values of points q and q + 1
+        // (not for 1024-point rows with global tables, where the packed loop makes ptxas spill: stream1024 +1 %)
+        constexpr bool PK = !HEAT && (TS || G >= 2);
+        if constexpr (PK) {
 #pragma unroll
-        for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
+            for (int q = 0; q < R; q += 2) {
+                own[M * q + m] = make_float2(v[q].x, v[q + 1].x);
+                own[M * (q + 1) + m] = make_float2(v[q].y, v[q + 1].y);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
+        }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
         SHG_WT(3);
 
@@ -550,7 +640,62 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             }
         };
         if constexpr (HEAT) { if (qrow) heat_half(true); }
-        if (P.nzt == 0) {
+        if constexpr (PK) {
+          // ---- two points per iteration in packed fp32x2 (rk4_point2): .x = point q, .y = point q + 1
+          auto finish2 = [&](int q, float2 a1x, float2 a1y, float2 a2x, float2 a2y) {
+              if (slot >= 0) {
+                  const float2 i1 = __fmul2_rn(__ffma2_rn(a1x, a1x, __fmul2_rn(a1y, a1y)), bc2(fsc));
+                  const float2 i2 = __fmul2_rn(__ffma2_rn(a2x, a2x, __fmul2_rn(a2y, a2y)), bc2(fsc));
+                  s1 += __float2ll_rn(i1.x) + __float2ll_rn(i1.y);
+                  s2 += __float2ll_rn(i2.x) + __float2ll_rn(i2.y);
+              }
+              p1[M * q] = a1x; p1[M * (q + 1)] = a1y;
+              p2[M * q] = a2x; p2[M * (q + 1)] = a2y;
+          };
+          if (P.nzt == 0) {
+            // uniform temperature: the step's coefficients from the table (warp-uniform 48-byte read)
+            PhaseCoef CA, CM, CB;
+            load_uniform_coefs(P, b, n, CA, CM, CB);
+            const PhaseCoef2 A2c = phase_coef2(CA), M2c = phase_coef2(CM), B2c = phase_coef2(CB);
+#pragma unroll 1
+            for (int q = 0; q < H; q += 2) {
+                float2 a1x = p1[M * q], a1y = ng2(p1[M * (q + 1)]);
+                float2 a2x = p2[M * q], a2y = ng2(p2[M * (q + 1)]);
+                rk4_point2(a1x, a1y, a2x, a2y, A2c, M2c, B2c, g1, g2);
+                finish2(q, a1x, a1y, a2x, a2y);
+            }
+          } else {
+            const float hdz = 0.5f * mb.dz, e8 = 0.125f * mb.dz;
+            const float gT = mb.gT, dk0 = mb.dk0, Thi = mb.Tpm_hi, Tlo = mb.Tpm_lo;
+#pragma unroll 1
+            for (int q = 0; q < H; q += 2) {
+                // consume the operands of points q, q + 1 (requested two points earlier), request those of q + 2, q + 3
+                const TPoint t0 = cur, t1 = nxt;
+                const int qa = (q + 2 < H) ? q + 2 : H - 1, qb = (q + 3 < H) ? q + 3 : H - 1;   // clamped tail
+                cur = t_load(Ta, Tn, plane, pbase + M * qa, ta.two, tb.two, phi + M * qa);
+                nxt = t_load(Ta, Tn, plane, pbase + M * qb, ta.two, tb.two, phi + M * qb);
+                const float2 dTa = dT_lerp2(make_float2(t0.a0, t1.a0), make_float2(t0.a1, t1.a1), ta.f, ta.two, Thi, Tlo);
+                const float2 dTb = dT_lerp2(make_float2(t0.b0, t1.b0), make_float2(t0.b1, t1.b1), tb.f, tb.two, Thi, Tlo);
+                const float2 dka = __ffma2_rn(bc2(gT), dTa, bc2(dk0)), dkb = __ffma2_rn(bc2(gT), dTb, bc2(dk0));
+                const float2 ph = make_float2(t0.ph, t1.ph);
+                const float2 phm = __ffma2_rn(bc2(e8), __ffma2_rn(bc2(3.0f), dka, dkb), ph);   // phi_n + dz (3 dk_n + dk_{n+1})/8
+                const float2 phb = __ffma2_rn(bc2(hdz), __fadd2_rn(dka, dkb), ph);             // phi_n + dz (dk_n + dk_{n+1})/2
+                float2 ca, sa, cm, sm, cb, sb;
+                __sincosf(ph.x, &sa.x, &ca.x);   __sincosf(ph.y, &sa.y, &ca.y);
+                __sincosf(phm.x, &sm.x, &cm.x);  __sincosf(phm.y, &sm.y, &cm.y);
+                __sincosf(phb.x, &sb.x, &cb.x);  __sincosf(phb.y, &sb.y, &cb.y);
+                const float2 pw = wrap_2pi2(phb);
+                __stcg(phi + M * q, pw.x);
+                __stcg(phi + M * (q + 1), pw.y);
+                const PhaseCoef2 CA = phase_coef2(ca, sa, k1dz, k2dz), CM = phase_coef2(cm, sm, k1dz, k2dz),
+                                 CB = phase_coef2(cb, sb, k1dz, k2dz);
+                float2 a1x = p1[M * q], a1y = ng2(p1[M * (q + 1)]);
+                float2 a2x = p2[M * q], a2y = ng2(p2[M * (q + 1)]);
+                rk4_point2(a1x, a1y, a2x, a2y, CA, CM, CB, g1, g2);
+                finish2(q, a1x, a1y, a2x, a2y);
+            }
+          }
+        } else if (P.nzt == 0) {
             // uniform temperature: the step's coefficients from the table (warp-uniform 48-byte read)
             PhaseCoef CA, CM, CB;
             load_uniform_coefs(P, b, n, CA, CM, CB);
@@ -621,8 +766,17 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
         SHG_WT(5);
+        if constexpr (PK) {
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
+            for (int q = 0; q < R; q += 2) {
+                const float2 re = own[M * q + m], im = own[M * (q + 1) + m];
+                v[q] = make_float2(re.x, im.x);
+                v[q + 1] = make_float2(re.y, im.y);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = own[M * q + m];
+        }
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
         SHG_WT(6);
