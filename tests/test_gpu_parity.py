@@ -725,10 +725,13 @@ def test_paper_ordering_launch_schemes_agree_and_argument_errors():
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,nz,kw", [("cfg2", 5, {}), ("cfg2", 5, {"scheme": 1}), ("cfg2", 6, {"heat": 4}),
                                         ("cfg3", 3, {}), ("cfg5", 3, {}), ("cfg4", 4, {"batch": 3}),
-                                        ("cfg2", 4, {"persistent": False, "scheme": 1}), ("cfg1", 4, {"heat": 1})])
+                                        ("cfg2", 4, {"persistent": False, "scheme": 1}), ("cfg1", 4, {"heat": 1}),
+                                        ("cfg4", 4, {"batch": 5, "pipeline": 2}), ("stream256", 3, {"batch": 3, "pipeline": 2}),
+                                        ("stream1024", 2, {"batch": 2, "pipeline": 2})])
 def test_no_access_outside_the_callers_arrays(name, nz, kw):
     kw = dict(kw)
     scheme, heat, persistent = kw.pop("scheme", 0), kw.pop("heat", 0), kw.pop("persistent", True)
+    pipeline = kw.pop("pipeline", 1)
     w = wl.make(name, nz=nz, **kw)
     g = dict(w["grid"])
     PAD = 4096                                                     # elements on either side (16-byte aligned)
@@ -742,6 +745,7 @@ def test_no_access_outside_the_callers_arrays(name, nz, kw):
     def run(guard):
         ctx = shg.Shg(g, w["crystal"], w["beams"], persistent=persistent)
         ctx.set_option(shg.OPT_SCHEME, scheme)
+        ctx.set_option(shg.OPT_PIPELINE, pipeline)                 # 2: the pipelined batched kernel (staged strips)
         keep = []
         nanc = complex(float("nan"), float("nan"))
         if g["nzt"] > 0:
