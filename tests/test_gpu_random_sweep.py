@@ -21,8 +21,10 @@ def rel(a, b):
     return float(np.linalg.norm((a - b).ravel()) / (nb if nb > 0 else 1.0))
 
 
-@pytest.mark.parametrize("seed", [11, 12, 13])
-def test_random_configurations_match_oracle(seed):
+@pytest.mark.parametrize("seed,pipe", [(11, False), (12, False), (13, False), (21, True), (22, True)])
+def test_random_configurations_match_oracle(seed, pipe):
+    """pipe: the same draws bent to batches of square grids in the pipelined batched kernel (SHG_OPT_PIPELINE = 2),
+    half of them with the temperature array handed over as a HOST array."""
     rng = np.random.default_rng(seed)
     for case in range(10):
         nx = int(rng.choice(SIZES, p=[0.35, 0.35, 0.2, 0.1]))
@@ -35,6 +37,12 @@ def test_random_configurations_match_oracle(seed):
         undep = bool(rng.random() < 0.2)
         persistent = bool(rng.random() < 0.6)
         nq = int(rng.integers(1, nz + 1)) if (rng.random() < 0.35 and scheme == 0) else 0
+        host_T = False
+        if pipe:
+            ny, scheme, nq, persistent = nx, 0, 0, True
+            batch = int(rng.integers(2, 6)) if nx <= 256 else 2
+            per_member = bool(rng.random() < 0.5) and nzt > 0
+            host_T = bool(rng.random() < 0.5)
         c = wl.crystal(float(rng.uniform(4e-3, 12e-3)), alpha=True, ddk_dT=float(rng.uniform(-400, 400)),
                        dk0=float(rng.uniform(-50, 50)), beta1=float(rng.choice([0.0, 2e-11])),
                        rho1=float(rng.choice([0.0, 1e-3])), rho2=float(rng.choice([0.0, -2e-3])))
@@ -56,8 +64,11 @@ def test_random_configurations_match_oracle(seed):
         ctx = shg.Shg(g, c, beams, persistent=persistent)
         ctx.set_option(shg.OPT_SCHEME, scheme)
         ctx.set_option(shg.OPT_UNDEPLETED, int(undep))
+        if pipe:
+            ctx.set_option(shg.OPT_PIPELINE, 2)
+            ctx.set_option(shg.OPT_CLUSTER, 0)
         if nzt > 0:
-            Td = torch.from_numpy(T).cuda()
+            Td = T if host_T else torch.from_numpy(T).cuda()
             ctx.set_temperature(Td, per_member=per_member)
         else:
             ctx.set_temperature(None, Tu)
@@ -67,6 +78,8 @@ def test_random_configurations_match_oracle(seed):
             ctx.set_heat_output(Q)
         g1, g2 = ctx.propagate(torch.from_numpy(A1).cuda(), None if A2 is None else torch.from_numpy(A2).cuda())
         torch.cuda.synchronize()
+        if pipe:
+            assert ctx.last_kernel() == 3, tag
 
         o = oracle.Oracle(g, c, beams, scheme=scheme, undepleted=undep)
         o.set_temperature(T, Tu, per_member)
