@@ -293,6 +293,10 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
     const float fsc = P.pfix[b];
     float phi[PT], dkn[PT], tq0[PT], tq1[PT];                       // phi(z_n), dk(z_n), raw T of the next node
     PhaseCoef CA[KP], CM[KP], CB[KP];
+    // PT == 2 (128 x 128): the thread's two points are integrated together in packed fp32x2 (rk4_point2: the same
+    // operations in the same order as the scalar code, see shg_device.cuh), their coefficients kept as pairs
+    constexpr bool PK2 = (PT == 2);
+    PhaseCoef2 CA2{}, CM2{}, CB2{};
 #pragma unroll
     for (int k = 0; k < PT; ++k) { phi[k] = 0.f; dkn[k] = 0.f; tq0[k] = 0.f; tq1[k] = 0.f; }
     auto point_row = [&](int k) {                                    // local row of point k
@@ -341,6 +345,24 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
                 s_coef[4] = c.u1x; s_coef[5] = c.u1y; s_coef[6] = c.u2x; s_coef[7] = c.u2y;
                 s_coef[8] = d.u1x; s_coef[9] = d.u1y; s_coef[10] = d.u2x; s_coef[11] = d.u2y;
             }
+        } else if constexpr (PK2) {
+            // both points at once (coefs_of_point, operation for operation, on pairs)
+            const TNode t = t_node(n + 1, P.nz, P.nzt);
+            const float2 dkb = __ffma2_rn(bc2(mb.gT), dT_lerp2(make_float2(tq0[0], tq0[PT - 1]), make_float2(tq1[0], tq1[PT - 1]),
+                                                                 t.f, t.two, mb.Tpm_hi, mb.Tpm_lo), bc2(mb.dk0));
+            const float2 ph = make_float2(phi[0], phi[PT - 1]), dka = make_float2(dkn[0], dkn[PT - 1]);
+            const float2 phm = __ffma2_rn(bc2(0.125f * mb.dz), __ffma2_rn(bc2(3.0f), dka, dkb), ph);
+            const float2 phb = __ffma2_rn(bc2(0.5f * mb.dz), __fadd2_rn(dka, dkb), ph);
+            float2 ca, sa, cm, sm, cb, sb;
+            __sincosf(ph.x, &sa.x, &ca.x);   __sincosf(ph.y, &sa.y, &ca.y);
+            __sincosf(phm.x, &sm.x, &cm.x);  __sincosf(phm.y, &sm.y, &cm.y);
+            __sincosf(phb.x, &sb.x, &cb.x);  __sincosf(phb.y, &sb.y, &cb.y);
+            const float2 pw = wrap_2pi2(phb);
+            phi[0] = pw.x; phi[PT - 1] = pw.y;
+            dkn[0] = dkb.x; dkn[PT - 1] = dkb.y;
+            CA2 = phase_coef2(ca, sa, k1dz, k2dz);
+            CM2 = phase_coef2(cm, sm, k1dz, k2dz);
+            CB2 = phase_coef2(cb, sb, k1dz, k2dz);
         } else if constexpr (PT <= 2) {
 #pragma unroll
             for (int k = 0; k < PT; ++k) coefs_of_point(k, dk_of(n + 1, k), CA[k], CM[k], CB[k]);
@@ -398,6 +420,34 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
         // ---- phase B (everyone): one RK4 step of Eq. 2 per point, power sums
         const int slot = rec_slot(P, n + 1);
         long long s1 = 0, s2 = 0;
+        if constexpr (PK2) {
+            float2* q1[2];
+            float2* q2[2];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const int idx = tid + k * THREADS;
+                const int li = idx / (HG * N), rw = (idx / N) % HG, e = idx % N;
+                q1[k] = scr + li * (G * NP) + rw * NP + e;
+                q2[k] = scr + li * (G * NP) + (HG + rw) * NP + ((e + N / 2) & (N - 1));
+            }
+            if (P.nzt == 0) {
+                CA2.u1x = bc2(s_coef[0]); CA2.u1y = bc2(s_coef[1]); CA2.u2x = bc2(s_coef[2]); CA2.u2y = bc2(s_coef[3]);
+                CM2.u1x = bc2(s_coef[4]); CM2.u1y = bc2(s_coef[5]); CM2.u2x = bc2(s_coef[6]); CM2.u2y = bc2(s_coef[7]);
+                CB2.u1x = bc2(s_coef[8]); CB2.u1y = bc2(s_coef[9]); CB2.u2x = bc2(s_coef[10]); CB2.u2y = bc2(s_coef[11]);
+            }
+            const float2 u0 = *q1[0], u1 = *q1[1], w0 = *q2[0], w1 = *q2[1];
+            float2 a1x = make_float2(u0.x, u1.x), a1y = make_float2(-u0.y, -u1.y);
+            float2 a2x = make_float2(w0.x, w1.x), a2y = make_float2(-w0.y, -w1.y);
+            rk4_point2(a1x, a1y, a2x, a2y, CA2, CM2, CB2, g1, g2);
+            *q1[0] = make_float2(a1x.x, a1y.x); *q1[1] = make_float2(a1x.y, a1y.y);
+            *q2[0] = make_float2(a2x.x, a2y.x); *q2[1] = make_float2(a2x.y, a2y.y);
+            if (slot >= 0) {
+                const float2 i1 = __fmul2_rn(__ffma2_rn(a1x, a1x, __fmul2_rn(a1y, a1y)), bc2(fsc));
+                const float2 i2 = __fmul2_rn(__ffma2_rn(a2x, a2x, __fmul2_rn(a2y, a2y)), bc2(fsc));
+                s1 = __float2ll_rn(i1.x) + __float2ll_rn(i1.y);
+                s2 = __float2ll_rn(i2.x) + __float2ll_rn(i2.y);
+            }
+        } else {
 #pragma unroll
         for (int k = 0; k < PT; ++k) {
             const int idx = tid + k * THREADS;
@@ -421,6 +471,7 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
                 s1 += to_fix(fmaf(a1.x, a1.x, a1.y * a1.y), fsc);
                 s2 += to_fix(fmaf(a2.x, a2.x, a2.y * a2.y), fsc);
             }
+        }
         }
         if (slot >= 0) {
             s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
