@@ -25,7 +25,8 @@
  *     phi, the power history and staging buffers, freed in shg_destroy.  They are allocated in shg_create,
  *     except: the device copy of a host temperature array (shg_set_temperature_host, on first use or growth),
  *     the two staging fields of shg_propagate_host (on its first call), the plane map of shg_set_heat_output
- *     and the trace buffer of SHG_OPT_TRACE.  shg_propagate (device pointers) allocates nothing.
+ *     and the trace buffer of SHG_OPT_TRACE.  shg_propagate (device pointers) allocates no memory; the first one
+ *     that uploads a large host temperature array creates the library's copy stream and its chunk events.
  *   - shg_propagate enqueues work on the given stream and returns without waiting.  shg_synchronize,
  *     shg_power and shg_power_history synchronise that stream and report a failed run (SHG_ECUDA).
  *   - Every call returns SHG_OK (0) or a negative code; nothing aborts or throws across the ABI.
