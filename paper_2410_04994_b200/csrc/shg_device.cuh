@@ -116,8 +116,17 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // to make room; chaining load k to product k - TABLE_DEPTH keeps TABLE_DEPTH loads in flight.  One LOP3 each.
 // Measured on cfg5 (us per z-step): depth 4: 40.2, 6: 39.0, 8: 39.1, 12: 36.6, 16: 36.7, 20: 38.7, 31 (no chain): 40.7
 // (spills return); the propagator tables are the sensitive ones (twiddles 6..16 with tables at 12-14: 36.6-37.8).
-constexpr int TABLE_DEPTH = 12;      // global propagator tables (L1 latency)
-constexpr int TWIDDLE_DEPTH = 12;    // shared-memory twiddles
+// Re-measured at the end of round 2 (radix-2^2 butterflies, packed RK4; -DSHG_TWIDDLE_DEPTH=d), cfg5 / cfg4 / stream256 /
+// stream1024: 4: 35.7 / 25.2 / 256 / 426, 8: 33.8 / 24.5 / 252 / 425, 10: 34.0 / 24.5 / 253 / 422, 12: 34.0 / 24.8 /
+// 252 / 421, 16: 34.2 / 24.5 / 251, 20: 34.1 / 24.4 / 250 -- flat within 1 % from 8 on; 12 stays.
+#ifndef SHG_TABLE_DEPTH
+#define SHG_TABLE_DEPTH 12
+#endif
+#ifndef SHG_TWIDDLE_DEPTH
+#define SHG_TWIDDLE_DEPTH 12
+#endif
+constexpr int TABLE_DEPTH = SHG_TABLE_DEPTH;      // global propagator tables (L1 latency)
+constexpr int TWIDDLE_DEPTH = SHG_TWIDDLE_DEPTH;  // shared-memory twiddles (and shared-memory propagator tables)
 
 template <int BYTE_OFF>
 __device__ __forceinline__ float4 lds128_after(unsigned saddr, float dep) {
