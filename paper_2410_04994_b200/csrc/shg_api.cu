@@ -239,7 +239,8 @@ struct shg_ctx {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t guard_ev = nullptr;
     std::vector<cudaEvent_t> up_ev;
-    int up_chunks = 0, up_planes = 0;    // chunks of the current upload, planes per chunk
+    int up_chunks = 0;                   // chunks of the current upload
+    std::vector<int> up_end;             // planes [0, up_end[c]) are on the device when chunk c has arrived
     const float* up_host = nullptr;      // deferred upload: the host array that the next propagate copies, chunk by chunk,
                                          // AFTER its own field uploads (the copy engine serves its queue in order)
 
@@ -631,10 +632,19 @@ static int enqueue_upload(shg_ctx* ctx, cudaStream_t st) {
     const size_t bytes = sizeof(float) * (size_t)nzt * plane_f;
     if (!ctx->copy_stream) CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
     if (!ctx->guard_ev) CU(cudaEventCreateWithFlags(&ctx->guard_ev, cudaEventDisableTiming));
-    int chunks = (int)(bytes >> 26);                           // ~64 MB each
+    int chunks = (int)(bytes >> 26);                           // ~64 MB each ...
     chunks = chunks < 2 ? 2 : (chunks > 16 ? 16 : chunks);
     const int planes = (nzt + chunks - 1) / chunks;
-    chunks = (nzt + planes - 1) / planes;
+    // ... after two small ones (1/8 and 1/4 of a chunk, at least two planes: a z-step needs two), so that the first
+    // launch of the z-loop waits for a few megabytes only
+    ctx->up_end.clear();
+    for (int p = 0, c = 0; p < nzt; ++c) {
+        int len = (c == 0) ? planes / 8 : (c == 1 ? planes / 4 : planes);
+        len = len < 2 ? 2 : len;
+        p = (p + len < nzt) ? p + len : nzt;
+        ctx->up_end.push_back(p);
+    }
+    chunks = (int)ctx->up_end.size();
     while ((int)ctx->up_ev.size() < chunks) {
         cudaEvent_t e;
         CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -647,13 +657,12 @@ static int enqueue_upload(shg_ctx* ctx, cudaStream_t st) {
         CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->guard_ev, 0));
     }
     for (int c = 0; c < chunks; ++c) {
-        const int p0 = c * planes, p1 = (p0 + planes < nzt) ? p0 + planes : nzt;
+        const int p0 = c ? ctx->up_end[(size_t)c - 1] : 0, p1 = ctx->up_end[(size_t)c];
         CU(cudaMemcpyAsync(ctx->d_T_owned + (size_t)p0 * plane_f, T_host + (size_t)p0 * plane_f,
                            sizeof(float) * (size_t)(p1 - p0) * plane_f, cudaMemcpyHostToDevice, ctx->copy_stream));
         CU(cudaEventRecord(ctx->up_ev[(size_t)c], ctx->copy_stream));
     }
     ctx->up_chunks = chunks;
-    ctx->up_planes = planes;
     return SHG_OK;
 }
 
@@ -881,7 +890,7 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
             // every launch).  The copy of chunk c + 1 runs under the z-steps of chunk c.
             int n0 = 0;
             for (int c = 0; c < ctx->up_chunks && n0 < g.nz; ++c) {
-                const int have = (c + 1) * ctx->up_planes < g.nzt ? (c + 1) * ctx->up_planes : g.nzt;   // planes [0, have)
+                const int have = ctx->up_end[(size_t)c];                   // planes [0, have) have arrived
                 int n1 = n0;
                 while (n1 < g.nz && last_plane_of_step(n1) < have) ++n1;
                 if (c == ctx->up_chunks - 1) n1 = g.nz;
