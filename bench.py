@@ -385,8 +385,9 @@ def run_b200(args):
         eta_map = gather_member_values(eta_local, total_members, rank, world)
 
     # ---- end to end through the host-buffer entry points: pinned host inputs -> device -> result on the host
-    e2e = None
-    if not args.no_e2e:
+    def time_e2e(ctx, w, g, B, stream, steps, warmup):
+        """ms for `steps` end-to-end steps (host temperature array + host fields in, fields + history out), and
+        the bytes moved per step."""
         hA1 = torch.from_numpy(w["A1"]).pin_memory()
         hO1, hO2 = torch.empty_like(hA1).pin_memory(), torch.empty_like(hA1).pin_memory()
         hT = torch.from_numpy(w["T"]).pin_memory() if g["nzt"] > 0 else None
@@ -401,19 +402,23 @@ def run_b200(args):
             ctx.propagate_host(hA1, None, hO1, hO2, stream=stream)
             return ctx.power_history(0)            # synchronises the stream and reads the history back
 
-        for _ in range(max(1, min(args.warmup, 2))):
+        for _ in range(warmup):
             e2e_step()
         barrier()
         t0 = time.perf_counter()
         ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
         ev2[0].record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             e2e_step()
         ev2[1].record(stream)
         barrier()
         wall_ms = (time.perf_counter() - t0) * 1e3
         # host work (history read-back) sits between device work, so take the larger of the two clocks
-        ms_e2e = max(ev2[0].elapsed_time(ev2[1]), wall_ms)
+        return max(ev2[0].elapsed_time(ev2[1]), wall_ms), h2d, d2h
+
+    e2e = None
+    if not args.no_e2e:
+        ms_e2e, h2d, d2h = time_e2e(ctx, w, g, B, stream, args.steps, max(1, min(args.warmup, 2)))
         t2 = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(t2, op=dist.ReduceOp.MAX)
@@ -468,8 +473,14 @@ def run_b200(args):
                 "roofline_frac": rf["frac"], "frac_of_distinct_operand_peak": rf["frac_of_distinct_operand_peak"],
                 "hbm_frac": rf["hbm"]["frac"], "two_pass_traffic_GBs": rf["hbm"]["two_pass_traffic_GBs"],
                 "gpu_launches_per_step": ro["launches"], "eta_member0": ro["ctx"].efficiency(0),
+                "e2e": None,
                 "clocks": {k: ck.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
             }
+            if not args.no_e2e:
+                # the same end-to-end measurement as the headline's, 1 warm-up + 2 timed steps
+                ms2, h2d_o, d2h_o = time_e2e(ro["ctx"], ro["w"], ro["g"], ro["B"], ro["stream"], 2, 1)
+                others[name]["e2e"] = {"value": ro["pts"] / (ms2 / 2 * 1e-3), "unit": UNIT, "ms_per_step": ms2 / 2,
+                                       "h2d_bytes_per_step": int(h2d_o), "d2h_bytes_per_step": int(d2h_o)}
             ro["ctx"].close()
             del ro
             torch.cuda.empty_cache()
