@@ -46,3 +46,30 @@ def gather_member_values(local: np.ndarray, n_members: int, rank: int, world: in
     outs = [torch.zeros(pad, dtype=torch.float64, device=dev) for _ in range(world)]
     dist.all_gather(outs, buf, group=group)
     return np.concatenate([o[:s].cpu().numpy() for o, s in zip(outs, sizes)])
+
+
+def sweep(w: dict, rank: int = 0, world: int = 1, group=None, options=None, stream=None) -> np.ndarray:
+    """A parameter sweep (BASELINE.json configs[3]; the paper runs one simulation per process): propagate
+    this rank's share of the members of the batched workload `w` (workloads.make output) in ONE launch sequence of
+    libshg and return the SH conversion efficiency P2(L) / (P1(0) + P2(0)) of EVERY member on every rank.
+    options: {shg.OPT_*: value}.  Needs the CUDA library; there is no other path."""
+    import torch
+    from . import shg
+    part = shard_workload(w, rank, world) if world > 1 else w
+    g = part["grid"]
+    ctx = shg.Shg(g, part["crystal"], part["beams"])
+    try:
+        for k, v in (options or {}).items():
+            ctx.set_option(k, v)
+        if g["nzt"] > 0:
+            T = part["T"]
+            ctx.set_temperature(T if isinstance(T, torch.Tensor) and T.is_cuda else torch.from_numpy(np.ascontiguousarray(T)).cuda(),
+                                per_member=part["per_member"])
+        else:
+            ctx.set_temperature(None, part["T_uniform"])
+        ctx.propagate(torch.from_numpy(np.ascontiguousarray(part["A1"])).cuda(), stream=stream)
+        ctx.synchronize()
+        local = np.array([ctx.efficiency(b) for b in range(g["batch"])])
+    finally:
+        ctx.close()
+    return gather_member_values(local, w["grid"]["batch"], rank, world, group)

@@ -350,6 +350,24 @@ def test_pipelined_kernel_at_scale_gives_the_same_bits(name, batch, nz, mode):
     assert np.isfinite(p1).all() and min(h[-1, 1] for h in ph) > 0
 
 
+def test_sweep_helper_returns_the_efficiency_map():
+    """sharding.sweep: the (xi, P) efficiency map of a batched workload in one call -- against the oracle on a
+    12-member corner of cfg4, and the shards of a two-rank split (run one after the other here) concatenate to it."""
+    from paper_2410_04994_b200 import sharding
+    w = wl.make("cfg4", nz=30, batch=12)
+    eta = sharding.sweep(w)
+    assert eta.shape == (12,)
+    o1, o2, oh = run_oracle(w)
+    eta_o = np.array([h[-1, 1] / (h[0, 0] + h[0, 1]) for h in oh])
+    assert np.max(np.abs(eta / eta_o - 1)) <= 1e-4
+    # (six members fit one wave of clusters, twelve do not: the cluster kernel's 128-point transform sums in another
+    # order than the batched kernels', so the shards agree with the whole to rounding, not bit for bit)
+    parts = [sharding.sweep(sharding.shard_workload(w, r, 2)) for r in range(2)]
+    assert np.allclose(np.concatenate(parts), eta, rtol=1e-5, atol=0)
+    same = [sharding.sweep(sharding.shard_workload(w, r, 2), options={shg.OPT_CLUSTER: 0}) for r in range(2)]
+    assert np.array_equal(np.concatenate(same), eta)
+
+
 def test_free_diffraction_matches_analytic_beam_on_gpu():
     """d_eff = 0: the GPU linear path alone against Eq. 5, no oracle involved."""
     n = 256
