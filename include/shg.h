@@ -46,6 +46,7 @@ extern "C" {
 #define SHG_ESTATE  (-2)   /* call made in the wrong state (temperature not set, power before run)   */
 #define SHG_ECUDA   (-3)   /* a CUDA call failed; shg_strerror(SHG_ECUDA) carries the CUDA message    */
 #define SHG_ENOMEM  (-4)   /* host or device allocation failed                                        */
+#define SHG_ELIMIT  (-5)   /* size beyond the fixed capacity of a static-scratch entry point          */
 
 typedef struct shg_ctx shg_ctx;   /* opaque, owned by the library */
 
@@ -232,6 +233,49 @@ int shg_last_cluster_size(const shg_ctx* ctx);
  * 2 = k_persist_flat (sparse launch), 3 = k_persist_pipe (SHG_OPT_PIPELINE), 4 = k_cluster, 5 = k_persist_paper
  * (SHG_OPT_SCHEME = 1).  Lets bench.py and the tests name what they measured. */
 int shg_last_kernel(const shg_ctx* ctx);
+
+/* The power integral for callers that must not allocate.
+ *
+ * Everything else in this header hangs off a context, and shg_create allocates device memory.  That rules the library
+ * out for code that runs where cudaMalloc / cudaFree may not be called: a hook inside another allocator or memory pool
+ * (an allocation there re-enters the pool or blocks on its lock), a plug-in whose host application owns all device
+ * memory and hands out fixed buffers, a latency-critical loop that cannot afford the driver's allocation lock or the
+ * device-wide wait inside cudaFree, a job sized to the last byte of HBM.  This one call needs no context and calls
+ * no cudaMalloc, cudaFree, nor any other routine that allocates:
+ *
+ *     P[b][j] = scale_j * sum over (iy, ix) of |A_j[b][iy][ix]|^2,   j = 1, 2,  b = 0 .. batch-1
+ *
+ * i.e. the power of both fields in W when scale_j = (eps0 c n_j / 2) dx dy -- the quantity shg_power reports at
+ * z = 0 for the inputs of a propagate, summed the same way (chunks of a member in double in a fixed order, then the
+ * chunk sums in chunk order: the result does not depend on scheduling and is the same bits on every call).
+ *
+ *   A1_device, A2_device  DEVICE complex fp32 [batch][ny][nx], 8-byte aligned, read only; A2_device may be NULL
+ *                         (then P[b][1] = 0).  nx, ny >= 1, any size (not only the powers of two of shg_grid).
+ *   P_device              DEVICE double [batch][2], 8-byte aligned, written by the kernel on `cuda_stream`; the caller
+ *                         owns it (and every other buffer) and reads it after synchronising the stream.
+ *   batch                 1 .. SHG_STATIC_MAX_BATCH.  More members than that: SHG_ELIMIT, nothing is enqueued --
+ *                         split the members over several calls.
+ *
+ * Where the scratch lives.  The chunk sums and the per-member tickets of the two-level sum sit in a fixed array of
+ * SHG_STATIC_SCRATCH_BYTES (257 KiB) inside the library's device image.  Every GPU on which the library is used holds
+ * that array from the moment the image is loaded there until the process exits, whether or not this call is used.
+ *
+ * First call on a device.  The first call made with a given device current looks up the array's address on that
+ * device (cudaGetSymbolAddress; this may also be what makes the CUDA runtime load the library's device image) and
+ * keeps it; later calls on that device only enqueue a 1 KiB memset of the tickets and one kernel.  Make that first
+ * call during set-up, with the right device current, and before you begin any stream capture on it.
+ *
+ * Sharing.  All calls on one device use the same array, and it keeps what the last call left in it (the call clears
+ * the part that must start at zero).  Two calls that can run on the GPU at the same time -- different streams without
+ * an event between them, or two host threads each with their own stream -- race on it and both results are
+ * undefined.  Calls on one stream, or ordered by events, are safe.
+ *
+ * Returns SHG_OK after enqueueing (it does not wait), SHG_EINVAL (NULL / misaligned pointer, size < 1), SHG_ELIMIT,
+ * or SHG_ECUDA (shg_strerror has the CUDA message). */
+#define SHG_STATIC_MAX_BATCH     256
+#define SHG_STATIC_SCRATCH_BYTES 263168
+int shg_field_power_static(const void* A1_device, const void* A2_device, int nx, int ny, int batch,
+                           double scale1, double scale2, double* P_device, void* cuda_stream);
 
 void shg_destroy(shg_ctx* ctx);
 

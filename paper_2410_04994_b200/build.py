@@ -59,8 +59,9 @@ def build(force: bool = False, verbose: bool = False, ptxas_info: bool = False) 
     for n in SIZES:
         o = os.path.join(OBJ, "shg_inst_%d.o" % n)
         jobs.append(([NVCC, *FLAGS, *extra, "-DSHG_N=%d" % n, "-c", os.path.join(CSRC, "shg_inst.cu"), "-o", o], o))
-    o = os.path.join(OBJ, "shg_api.o")
-    jobs.append(([NVCC, *FLAGS, *extra, "-c", os.path.join(CSRC, "shg_api.cu"), "-o", o], o))
+    for name in ("shg_api", "shg_static"):
+        o = os.path.join(OBJ, name + ".o")
+        jobs.append(([NVCC, *FLAGS, *extra, "-c", os.path.join(CSRC, name + ".cu"), "-o", o], o))
     logs = []
     with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
         for out in ex.map(lambda j: _run(j[0], verbose), jobs):

@@ -425,6 +425,8 @@ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 
 }  // namespace
 
+int shg::record_cuda_error(cudaError_t e, const char* what) { return cuda_fail(e, what); }
+
 extern "C" {
 
 const char* shg_strerror(int code) {
@@ -434,6 +436,9 @@ const char* shg_strerror(int code) {
         case SHG_ESTATE: return "call made in the wrong state (temperature not set, or power requested before a propagate)";
         case SHG_ECUDA: return g_cuda_msg.c_str();
         case SHG_ENOMEM: return "allocation failed";
+        case SHG_ELIMIT:
+            return "size beyond the fixed capacity of an entry point that works in static scratch "
+                   "(shg_field_power_static: at most SHG_STATIC_MAX_BATCH = 256 members per call)";
         default: return "unknown error code";
     }
 }

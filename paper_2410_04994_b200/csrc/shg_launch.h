@@ -26,6 +26,10 @@ struct LaunchInfo {
                                    cudaStream_t st);                                                        \
     LaunchInfo launch_info_##N();
 
+// Records a failed CUDA call as the message behind shg_strerror(SHG_ECUDA) and returns SHG_ECUDA (shg_api.cu);
+// lets the other translation units of the library (shg_static.cu) report through the same channel.
+int record_cuda_error(cudaError_t e, const char* what);
+
 SHG_DECLARE_N(64)
 SHG_DECLARE_N(128)
 SHG_DECLARE_N(256)

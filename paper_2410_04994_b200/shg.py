@@ -14,7 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libshg.so")
 
-SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM = 0, -1, -2, -3, -4
+SHG_OK, SHG_EINVAL, SHG_ESTATE, SHG_ECUDA, SHG_ENOMEM, SHG_ELIMIT = 0, -1, -2, -3, -4, -5
+STATIC_MAX_BATCH = 256          # SHG_STATIC_MAX_BATCH
 OPT_PERSISTENT, OPT_PRECISE, OPT_TRACE, OPT_ACQUIRE_FENCE, OPT_UNDEPLETED, OPT_SCHEME = 1, 2, 3, 4, 5, 6
 OPT_SPIN_LIMIT, OPT_TABLES_SMEM, OPT_CLUSTER, OPT_PIPELINE = 7, 8, 9, 10
 
@@ -22,7 +23,8 @@ EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_tempe
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
            "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
            "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
-           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct", "shg_last_kernel")
+           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct", "shg_last_kernel",
+           "shg_field_power_static")
 
 
 class Grid(C.Structure):
@@ -79,6 +81,7 @@ def lib():
     L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
     L.shg_measure_fp32_peak.argtypes = [dp]
     L.shg_measure_fp32_peak_distinct.argtypes = [dp]
+    L.shg_field_power_static.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp, vp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
     L.shg_strerror.argtypes = [C.c_int]
@@ -130,6 +133,30 @@ def measure_fp32_peak_distinct() -> float:
     v = C.c_double()
     _check(lib().shg_measure_fp32_peak_distinct(C.byref(v)))
     return float(v.value)
+
+
+def field_power_static(A1, A2, scale1: float, scale2: float, out, stream=None):
+    """shg_field_power_static: out[b][j] = scale_j * sum |A_j[b]|^2 with no context and no allocation.
+
+    For callers that may not allocate device memory (code running inside another allocator, a host application that
+    owns all of HBM, a loop that cannot take the driver's allocation lock): this wrapper allocates nothing either, so
+    the caller passes every buffer.  A1, A2 (or None): CUDA complex64 [batch][ny][nx]; out: CUDA float64 [batch][2],
+    written on `stream` (default: torch's current stream) -- synchronise before reading it.  batch is at most
+    STATIC_MAX_BATCH; beyond it the call raises ShgError (SHG_ELIMIT) and enqueues nothing.  All calls on a device
+    share one fixed scratch array inside the library: do not let two of them overlap on the GPU.  The first call on
+    a device looks the array up; make it before any stream capture.  See include/shg.h.
+    """
+    if A1.dim() != 3:
+        raise ValueError("A1 must be [batch][ny][nx]")
+    batch, ny, nx = A1.shape
+    if A2 is not None and tuple(A2.shape) != tuple(A1.shape):
+        raise ValueError("A2 must have the shape of A1")
+    if out.numel() != 2 * batch:
+        raise ValueError("out must hold batch*2 float64 values")
+    _check(lib().shg_field_power_static(_dev_ptr(A1, ("complex64",)), _dev_ptr(A2, ("complex64",)), nx, ny, batch,
+                                        float(scale1), float(scale2), _dev_ptr(out, ("float64",)),
+                                        _stream_ptr(stream)))
+    return out
 
 
 class Shg:
