@@ -123,7 +123,13 @@ typedef struct {
                                   transform's transposition as bulk asynchronous copies between the CTAs' shared
                                   memories signalled on mbarriers, no device-wide barrier; 0: never; 8 or 16: that
                                   cluster size whenever the grid size allows, even if the clusters run in several
-                                  waves.  Same arithmetic as the other kernels: bit-identical fields and powers.   */
+                                  waves.  64-point lines use the other kernels' line transform: bit-identical fields
+                                  and powers.  128-point lines are transformed over twice the lanes, in another
+                                  summation order: fields and powers agree with the other kernels to fp32 rounding
+                                  (rel. L2 ~1e-6 per propagate, tested < 2e-6), NOT bit for bit.  Since mode 1 picks
+                                  the kernel from the batch size and from how many clusters the device can hold, the
+                                  last bits of a 128 x 128 member may differ between a single run and the same member
+                                  inside a large batch; set 0 where bit-reproducibility across batch sizes matters.  */
 
 #define SHG_OPT_PIPELINE   10   /* batched runs (batch >= 2) in the persistent kernel.  The members are split into
                                   two groups whose row and column phases interleave, every device-wide barrier is
@@ -187,7 +193,8 @@ int shg_synchronize(shg_ctx* ctx);
 /* Power (W) of both fields of `member` at the RECORDED node nearest to z (step nodes z_n = n L/nz; recorded:
  * shg_grid.record_every).  The SH efficiency is derived by the caller: eta = P2(L) / (P1(0) + P2(0))  (P:288,
  * G16).  The sums behind these numbers are accumulated in fixed point (integers): they are bit-reproducible
- * from run to run and identical between launch schemes. */
+ * from run to run, and identical between launch schemes whose fields are identical (all of them except the cluster
+ * kernel on 128-point lines, see SHG_OPT_CLUSTER). */
 int shg_power(shg_ctx* ctx, int member, double z, double* P1, double* P2);
 
 /* Number of recorded nodes (ceil(nz / record_every) + 1), and their step indices n (HOST int32 array of that
