@@ -362,6 +362,8 @@ def run_b200(args):
     # collective; weak scaling).  --shard-members: the members of a sweep are split over the ranks (strong
     # scaling), the efficiency map is gathered at the end.  DESIGN.md 8.
     shard = args.shard_members and world > 1
+    if shard and wl.make(args.workload, nz=1)["grid"]["batch"] < world:
+        raise SystemExit("bench.py --shard-members: %s has fewer members than ranks (%d)" % (args.workload, world))
     sampler = ClockSampler(local).start() if rank == 0 else None
     r = time_workload(args.workload, args.steps, args.warmup, args, barrier, nz=args.nz,
                       members=(rank, world) if shard else None)

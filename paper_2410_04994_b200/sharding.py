@@ -48,14 +48,10 @@ def gather_member_values(local: np.ndarray, n_members: int, rank: int, world: in
     return np.concatenate([o[:s].cpu().numpy() for o, s in zip(outs, sizes)])
 
 
-def sweep(w: dict, rank: int = 0, world: int = 1, group=None, options=None, stream=None) -> np.ndarray:
-    """A parameter sweep (BASELINE.json configs[3]; the paper runs one simulation per process, P:256): propagate
-    this rank's share of the members of the batched workload `w` (workloads.make output) in ONE launch sequence of
-    libshg and return the SH conversion efficiency P2(L) / (P1(0) + P2(0)) of EVERY member on every rank.
-    options: {shg.OPT_*: value}.  Needs the CUDA library; there is no other path."""
+def _member_efficiencies(part: dict, options=None, stream=None) -> np.ndarray:
+    """Propagate the members of `part` on the current CUDA device and return their SH conversion efficiencies."""
     import torch
     from . import shg
-    part = shard_workload(w, rank, world) if world > 1 else w
     g = part["grid"]
     ctx = shg.Shg(g, part["crystal"], part["beams"])
     try:
@@ -67,9 +63,26 @@ def sweep(w: dict, rank: int = 0, world: int = 1, group=None, options=None, stre
                                 per_member=part["per_member"])
         else:
             ctx.set_temperature(None, part["T_uniform"])
-        ctx.propagate(torch.from_numpy(np.ascontiguousarray(part["A1"])).cuda(), stream=stream)
+        A1 = torch.from_numpy(np.ascontiguousarray(part["A1"])).cuda()
+        if stream is not None:
+            # the uploads above ran on torch's current stream: the propagate on `stream` must come after them
+            stream.wait_stream(torch.cuda.current_stream())
+        ctx.propagate(A1, stream=stream)
         ctx.synchronize()
-        local = np.array([ctx.efficiency(b) for b in range(g["batch"])])
+        return np.array([ctx.efficiency(b) for b in range(g["batch"])])
     finally:
         ctx.close()
+
+
+def sweep(w: dict, rank: int = 0, world: int = 1, group=None, options=None, stream=None) -> np.ndarray:
+    """A parameter sweep (BASELINE.json configs[3]; the paper runs one simulation per process, P:256): propagate
+    this rank's share of the members of the batched workload `w` (workloads.make output) in ONE launch sequence of
+    libshg and return the SH conversion efficiency P2(L) / (P1(0) + P2(0)) of EVERY member on every rank.
+    options: {shg.OPT_*: value}.  A rank whose share is empty (fewer members than ranks) propagates nothing and
+    still takes part in the gather.  Needs the CUDA library; there is no other path."""
+    part = shard_workload(w, rank, world) if world > 1 else w
+    if part["grid"]["batch"] == 0:
+        local = np.empty(0, dtype=np.float64)
+    else:
+        local = _member_efficiencies(part, options, stream)
     return gather_member_values(local, w["grid"]["batch"], rank, world, group)

@@ -107,6 +107,17 @@ assert mine["A1"].shape[0] == len(member_range(7, rank, world)) == mine["grid"][
 local = np.array([b["P"] for b in mine["beams"]])
 full = gather_member_values(local, 7, rank, world)
 assert np.allclose(full, [b["P"] for b in w["beams"]]), full
+# fewer members than ranks: the rank with the empty share creates no context and still joins the gather
+# (the propagation itself is stood in for: this box has no GPU)
+from paper_2410_04994_b200 import sharding
+w1 = wl.make("cfg4", nz=2, batch=1)
+assert shard_workload(w1, 1, world)["grid"]["batch"] == 0
+def stand_in(part, options=None, stream=None):
+    assert part["grid"]["batch"] > 0, "an empty share must not reach the library"
+    return np.array([b["P"] for b in part["beams"]])
+sharding._member_efficiencies = stand_in
+full = sharding.sweep(w1, rank, world)
+assert full.shape == (1,) and full[0] == w1["beams"][0]["P"], full
 dist.barrier()
 dist.destroy_process_group()
 print("ok", rank)
