@@ -64,17 +64,26 @@ def measured_peak_hbm():
 
 
 def ncu_traffic_bytes(workload: str, nz: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed
-    ncu --set full summary (profiles/roofline_traffic.csv: workload,nz,kernel,dram_bytes_per_launch)."""
+    """(bytes, source): dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
+    committed ncu capture (profiles/roofline_traffic.csv: workload,nz,kernel,dram_bytes_per_launch,kernel_digest).
+    A row counts only when its digest is the one of the device code being timed (build.kernel_digest()): a capture
+    of other code gives bytes = None."""
+    from paper_2410_04994_b200 import build as shg_build
     p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if not os.path.exists(p):
-        return None
+        return None, "no capture (profiles/roofline_traffic.csv is missing)"
+    dig = shg_build.kernel_digest()
     for line in open(p):
         f = [s.strip() for s in line.split(",")]
         if len(f) >= 4 and f[0] == workload and f[1].isdigit():
+            if len(f) < 5 or f[4] != dig:
+                return None, ("stale: the capture in profiles/roofline_traffic.csv is of kernel sources %s, this build "
+                              "is %s" % (f[4] if len(f) >= 5 else "without a digest", dig))
             # scale linearly in the z-step count when the capture used a shorter run of the same kernel
-            return float(f[3]) * nz / int(f[1])
-    return None
+            return float(f[3]) * nz / int(f[1]), (
+                "static: ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel in the capture committed as "
+                "profiles/roofline_traffic.csv (same kernel sources, digest %s; not re-measured in this run)" % dig)
+    return None, "no capture of this workload in profiles/roofline_traffic.csv"
 
 
 class ClockSampler:
@@ -314,9 +323,7 @@ def roofline_of(r, fp32_measured, fp32_distinct, traffic):
     achieved = b_alg * pts / t_loop / 1e9
     return {
         "bound": "alu", "achieved": achieved_tf, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-        "frac": achieved_tf / FP32_PEAK_TFLOPS, "traffic": traffic,
-        "traffic_source": "static: ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel in the capture "
-                          "committed as profiles/roofline_traffic.csv (not re-measured in this run)",
+        "frac": achieved_tf / FP32_PEAK_TFLOPS, "traffic": traffic[0], "traffic_source": traffic[1],
         "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 flops x 1.965 GHz (DESIGN.md 7)",
         "kernel": r["kernel"], "kernel_ms_per_launch": r["main_loop_ms"],
         "us_per_z_step": 1e3 * r["main_loop_ms"] / r["g"]["nz"],
@@ -435,8 +442,9 @@ def run_b200(args):
         return 0
 
     # ---- roofline of the dominant kernel (the z-loop kernel: k_persist / k_cluster, or the k_row/k_col pairs)
-    fp32_measured = shg.measure_fp32_peak()             # register-only FFMA kernel, CUDA events
-    fp32_distinct = shg.measure_fp32_peak_distinct()
+    from paper_2410_04994_b200 import diag              # libshg_diag.so: measuring equipment, not the product library
+    fp32_measured = diag.measure_fp32_peak()            # register-only FFMA kernel, CUDA events
+    fp32_distinct = diag.measure_fp32_peak_distinct()
     roofline = roofline_of(r, fp32_measured, fp32_distinct, ncu_traffic_bytes(w["name"], g["nz"]))
 
     cpu = None

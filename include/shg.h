@@ -99,9 +99,10 @@ typedef struct {
 #define SHG_OPT_ACQUIRE_FENCE 4 /* persistent kernel, acquire side of the device-wide barrier.  2 (default): the poll
                                   ends with an ld.acquire.gpu of the barrier counter (pairs with the arrivals'
                                   red.release.gpu; conforms to the PTX memory model); 1: a gpu-scope fence.acq_rel
-                                  after a relaxed poll (same guarantee); 0: no acquire at all -- the fields are read
-                                  with L2-only loads (ld.global.cg), which works on sm_100a but is outside the
-                                  memory model; kept for measurements.  Bit-identical results in all modes.        */
+                                  after a relaxed poll (same guarantee).  Bit-identical results in both modes.  (0, no
+                                  acquire at all with the fields read by L2-only loads, is outside the memory model
+                                  and is refused with SHG_EINVAL unless the library is built with
+                                  -DSHG_ALLOW_UNFENCED for a measurement; DESIGN.md 5.5 has round 2's numbers.)       */
 #define SHG_OPT_UNDEPLETED 5    /* 1: drop the coupling term of dA1/dz (the pump only diffracts and is absorbed), the
                                   "dPump = 0" check against Boyd-Kleinman of P:292; 0 (default): full Eq. 2.       */
 #define SHG_OPT_SCHEME     6    /* 0 (default): L/2 - N(dz) - L/2 with neighbouring half-steps merged (north_star);
@@ -151,12 +152,15 @@ int shg_set_option(shg_ctx* ctx, int option, int value);
 int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, int per_member);
 
 /* Same, from a HOST array: copied (asynchronously when the memory is pinned) into a library-owned device buffer that is
- * allocated on first use and reused afterwards.  A small array is copied on `cuda_stream` right away.  One array
- * shared by all members of 32 MB or more is uploaded by the NEXT shg_propagate[_host] instead, in chunks of planes on
+ * allocated on first use and reused afterwards.  An array in pageable memory, and any small array, is copied on
+ * `cuda_stream` during the call: the caller may free or reuse a pageable buffer as soon as the call returns.  One array
+ * shared by all members of 32 MB or more in PAGE-LOCKED memory (cudaMallocHost / cudaHostRegister / managed) is
+ * uploaded by the NEXT shg_propagate[_host] instead, in chunks of planes on
  * the library's own copy stream, behind that call's field uploads: the persistent kernel of a single simulation is
  * launched once per chunk, over the z-steps whose planes the chunk completes (a z-step reads only the planes around
  * its two nodes), so the transfer of chunk c + 1 runs under the z-steps of chunk c; every other kernel waits for the
- * last chunk.  T_host must therefore stay valid and unchanged until that propagate has completed. */
+ * last chunk.  A page-locked T_host must therefore stay valid and unchanged until that propagate has completed (as any
+ * buffer handed to an asynchronous copy must). */
 int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform, int per_member,
                              void* cuda_stream);
 
@@ -187,7 +191,10 @@ int shg_set_heat_output(shg_ctx* ctx, float* Q_device, int nq);
 
 /* Wait for the last propagate of this context and report how it ended: SHG_OK, or SHG_ECUDA when the stream
  * failed or a device-wide barrier of the persistent kernel timed out (the outputs are then invalid).  Call it
- * (or shg_power*) before trusting A1_out / A2_out of a run whose history you do not read. */
+ * (or shg_power*) before trusting A1_out / A2_out of a run whose history you do not read.  The timeout flag is
+ * sticky: it survives later propagates of the context (whose kernels then stop at their first barrier) and is cleared
+ * only by the call that reports it, so the error covers every propagate enqueued since the last successful
+ * shg_synchronize / shg_power*. */
 int shg_synchronize(shg_ctx* ctx);
 
 /* Power (W) of both fields of `member` at the RECORDED node nearest to z (step nodes z_n = n L/nz; recorded:
@@ -220,15 +227,6 @@ int shg_last_main_loop_ms(shg_ctx* ctx, float* ms);
  * out: HOST int64 [*steps][*grid][2][4] (see SHG_OPT_TRACE); out == NULL only queries *steps and *grid.
  * Synchronises the stream of the last propagate. */
 int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid);
-
-/* Measured fp32 pipe peak of the current device: a register-only FFMA kernel (16 independent chains per
- * thread, 512 threads per SM) timed with CUDA events.  *tflops receives 2 flops per FFMA lane-op over the
- * elapsed time.  It is the denominator of bench.py's "alu" roofline (nominal: SMs x 128 lanes x 2 x clock). */
-int shg_measure_fp32_peak(double* tflops);
-
-/* The same measurement with three distinct register operands per FFMA (no operand reuse between neighbouring
- * instructions), which is what the butterflies and the RK4 stages of this library look like to the register file. */
-int shg_measure_fp32_peak_distinct(double* tflops);
 
 /* Number of kernels the last shg_propagate / shg_propagate_host launched. */
 int shg_last_launch_count(const shg_ctx* ctx);

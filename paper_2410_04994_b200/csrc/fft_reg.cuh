@@ -101,42 +101,15 @@ __device__ __forceinline__ float2 twmul32(float2 d) {
     }
 }
 
-// one decimation-in-frequency butterfly of span SPAN: (a, b) -> (a + b, (a - b) w)
-template <int R, int SPAN, int J, bool INV, bool PREC>
-__device__ __forceinline__ void dif_bfly(float2 (&v)[R]) {
-    constexpr int grp = J / SPAN, k = J % SPAN;
-    constexpr int i0 = grp * 2 * SPAN + k, i1 = i0 + SPAN;
-    constexpr int E = k * (16 / SPAN);       // W_{2 SPAN}^k = W_32^{k 16/SPAN}
-    float2 a = v[i0], b = v[i1];
-    // Blackwell packed fp32x2 adds (FADD2: one issue slot for the re and im lanes of a register pair; the
-    // negation is an operand modifier).  The -i twiddle swaps re and im, which a register pair cannot do for
-    // free, so that difference stays scalar (its swap is then just register naming).
-    v[i0] = __fadd2_rn(a, b);
-    if constexpr (E == 8) v[i1] = twmul32<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));
-    else v[i1] = twmul32<E, INV, PREC>(__fadd2_rn(a, make_float2(-b.x, -b.y)));
-}
-
-template <int R, int SPAN, bool INV, bool PREC, int... J>
-__device__ __forceinline__ void dif_stage(float2 (&v)[R], std::integer_sequence<int, J...>) {
-    (dif_bfly<R, SPAN, J, INV, PREC>(v), ...);
-}
-
-template <int R, int SPAN, bool INV, bool PREC>
-__device__ __forceinline__ void dif_stages(float2 (&v)[R]) {
-    if constexpr (SPAN >= 1) {
-        dif_stage<R, SPAN, INV, PREC>(v, std::make_integer_sequence<int, R / 2>{});
-        dif_stages<R, SPAN / 2, INV, PREC>(v);
-    }
-}
-
-// ---- radix-2^2 arrangement of the same butterflies -------------------------------------------------------------
-// The decimation-in-frequency network above multiplies by W_{2 SPAN}^k after EVERY stage (32 points: 20 general
+// ---- radix-2^2 arrangement of the radix-2 butterflies ----------------------------------------------------------
+// The plain decimation-in-frequency network (round 1) multiplies by W_{2 SPAN}^k after EVERY stage (32 points: 20 general
 // and 14 eighth-root twiddles).  Moving the twiddles of two consecutive stages behind the second one (He &
 // Torkelson's radix-2^2: the first stage of a pair keeps only the factor -i on the upper half of its differences,
 // the second stage none, then the outputs of the length-4S block are multiplied by W_{4S}^{k j}, j = 0, 2, 1, 3 for its
 // four quarters) leaves the butterfly topology and the bit-reversed output order unchanged and needs 16 general + 12
 // eighth-root twiddles per 32 points (16 points: 4 + 4 instead of 4 + 6).  The transforms run at the fp32 pipe's
-// throughput (tests/probes/fft_issue_rate.cu), so the saved operations are saved time.
+// throughput (measured by a stand-alone issue-rate probe, profiles/r02b_fft_issue_rate.txt), so the saved operations
+// are saved time.
 
 // d * W_32^E (fwd; conj for INV) for E = 0..31: E >= 16 is the negative of E - 16 (folded into the constants)
 template <int E, bool INV, bool PREC>
@@ -158,7 +131,7 @@ template <int R, int I0, int I1, int E, bool INV, bool PREC>
 __device__ __forceinline__ void bfly_tw(float2 (&v)[R]) {
     const float2 a = v[I0], b = v[I1];
     v[I0] = __fadd2_rn(a, b);
-    if constexpr (E % 16 == 8) v[I1] = twmul32x<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));   // (+-i: scalar, see dif_bfly)
+    if constexpr (E % 16 == 8) v[I1] = twmul32x<E, INV, PREC>(make_float2(a.x - b.x, a.y - b.y));   // (+-i swaps re and im, which a register pair cannot do for free: scalar)
     else v[I1] = twmul32x<E, INV, PREC>(__fadd2_rn(a, make_float2(-b.x, -b.y)));
 }
 // (a, b) -> (a + b) * W_32^E0 and (a - b) * W_32^E1
@@ -219,11 +192,7 @@ __device__ __forceinline__ void brev_all(float2 (&v)[R], std::integer_sequence<i
 template <int R, bool INV, bool PREC>
 __device__ __forceinline__ void fft_reg(float2 (&v)[R]) {
     static_assert(R == 2 || R == 4 || R == 8 || R == 16 || R == 32, "radix");
-#ifdef SHG_FFT_RADIX2
-    dif_stages<R, R / 2, INV, PREC>(v);
-#else
     r22<R, 0, R, INV, PREC>(v);
-#endif
     brev_all<R>(v, std::make_integer_sequence<int, R>{});
 }
 

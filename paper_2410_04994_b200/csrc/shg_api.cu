@@ -134,52 +134,17 @@ __global__ void __launch_bounds__(256) k_input_power(const float2* __restrict__ 
     }
 }
 
-// nzt == 0: coupling coefficients of every (member, z-step), see shg_device.cuh: uniform_coefs
-__global__ void k_uniform_coefs(const shg::MemberDev* mem, float4* ucoef, int nz, int batch) {
+// nzt == 0: coupling coefficients of every z-step, see shg_device.cuh: uniform_coefs.  One table for all members (the
+// quantities that enter are the crystal's and T_uniform, identical in every MemberDev): member 0's scalars are used.
+__global__ void k_uniform_coefs(const shg::MemberDev* mem, float4* ucoef, int nz) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nz * batch) return;
-    const int b = i / nz, n = i - b * nz;
+    if (i >= nz) return;
+    const int n = i;
     shg::PhaseCoef a, c, d;
-    shg::uniform_coefs(mem[b], n, a, c, d);
+    shg::uniform_coefs(mem[0], n, a, c, d);
     ucoef[(size_t)i * 3 + 0] = make_float4(a.u1x, a.u1y, a.u2x, a.u2y);
     ucoef[(size_t)i * 3 + 1] = make_float4(c.u1x, c.u1y, c.u2x, c.u2y);
     ucoef[(size_t)i * 3 + 2] = make_float4(d.u1x, d.u1y, d.u2x, d.u2y);
-}
-
-// fp32 pipe peak: 16 independent FFMA chains per thread, nothing else in the loop
-__global__ void __launch_bounds__(512, 1) k_fp32_peak(float* out, const float* in, int iters) {
-    float a[16];
-    const float b = in[threadIdx.x & 31], c = in[32 + (threadIdx.x & 31)];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) a[i] = in[i] + (float)threadIdx.x;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], b, c);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += a[i];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-// the same with three DISTINCT register operands per FFMA (no operand reuse between neighbouring instructions): what
-// a transform butterfly or an RK4 stage looks like to the register file
-__global__ void __launch_bounds__(512, 1) k_fp32_peak_distinct(float* out, const float* in, int iters) {
-    float a[16], b[16], c[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        a[i] = in[i] + (float)threadIdx.x;
-        b[i] = in[16 + i] + 1.0f;
-        c[i] = in[32 + i];
-    }
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], b[i], c[i]);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += a[i];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
 }  // namespace
@@ -211,7 +176,7 @@ struct shg_ctx {
     float4* d_hy[2] = {nullptr, nullptr};
     shg::MemberDev* d_mem = nullptr;
     shg::GaussDev* d_gauss = nullptr;
-    float4* d_ucoef = nullptr;           // nzt == 0: [batch][nz][3] coupling coefficients per z-step
+    float4* d_ucoef = nullptr;           // nzt == 0: [nz][3] coupling coefficients per z-step, shared by all members
     float* d_phi = nullptr;
     long long* d_hfix = nullptr;         // [batch][nrec+1][2] fixed-point power sums
     float* d_pfix = nullptr;             // [batch] fixed-point scale 2^e of each member
@@ -372,8 +337,7 @@ int upload_tables(shg_ctx* ctx) {
     CU(cudaMemcpy(ctx->d_mem, mem.data(), sizeof(shg::MemberDev) * B, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_gauss, gs.data(), sizeof(shg::GaussDev) * B, cudaMemcpyHostToDevice));
     if (ctx->d_ucoef) {
-        const int total = g.nz * B;
-        k_uniform_coefs<<<(total + 127) / 128, 128>>>(ctx->d_mem, ctx->d_ucoef, g.nz, B);
+        k_uniform_coefs<<<(g.nz + 127) / 128, 128>>>(ctx->d_mem, ctx->d_ucoef, g.nz);
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(nullptr));
     }
@@ -491,7 +455,7 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     alloc((void**)&ctx->d_mem, sizeof(shg::MemberDev) * B);
     alloc((void**)&ctx->d_gauss, sizeof(shg::GaussDev) * B);
     if (grid->nzt > 0) alloc((void**)&ctx->d_phi, sizeof(float) * (size_t)B * np);
-    else alloc((void**)&ctx->d_ucoef, sizeof(float4) * (size_t)B * grid->nz * 3);
+    else alloc((void**)&ctx->d_ucoef, sizeof(float4) * (size_t)grid->nz * 3);
     alloc((void**)&ctx->d_hfix, sizeof(long long) * (size_t)B * (ctx->nrec + 1) * 2);
     alloc((void**)&ctx->d_pfix, sizeof(float) * B);
     alloc((void**)&ctx->d_inpart, sizeof(double) * (size_t)B * 64 * 2);
@@ -499,6 +463,9 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
     alloc((void**)&ctx->d_barrier, 8 * sizeof(unsigned int));
     if (!ok) { free_ctx(ctx); return SHG_ECUDA; }
     e = cudaMemset(ctx->d_ticket, 0, sizeof(unsigned int) * B);
+    if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaMemset"); }
+    // the status word [1] is cleared here and by the call that reports it, never by a propagate (it is sticky)
+    e = cudaMemset(ctx->d_barrier, 0, 8 * sizeof(unsigned int));
     if (e != cudaSuccess) { free_ctx(ctx); return cuda_fail(e, "cudaMemset"); }
     ctx->hist_host.assign((size_t)B * (ctx->nrec + 1) * 2, 0.0);
     ctx->hfix_host.assign((size_t)B * (ctx->nrec + 1) * 2, 0);
@@ -516,7 +483,13 @@ int shg_set_option(shg_ctx* ctx, int option, int value) {
     switch (option) {
         case SHG_OPT_PERSISTENT: ctx->persistent = (value != 0); return SHG_OK;
         case SHG_OPT_ACQUIRE_FENCE:
+            // 0 (no acquire at all) is outside the PTX memory model: not in the product build; -DSHG_ALLOW_UNFENCED
+            // brings it back for a measurement
+#ifdef SHG_ALLOW_UNFENCED
             if (value < 0 || value > 2) return SHG_EINVAL;
+#else
+            if (value < 1 || value > 2) return SHG_EINVAL;
+#endif
             ctx->acquire_fence = value;
             return SHG_OK;
         case SHG_OPT_SPIN_LIMIT:
@@ -595,7 +568,18 @@ int shg_set_temperature_host(shg_ctx* ctx, const float* T_host, double T_uniform
     const int nzt = ctx->g.nzt;
     ctx->up_chunks = 0;
     ctx->up_host = nullptr;
-    if (!(per_member && ctx->g.batch > 1) && nzt >= 8 && bytes >= ((size_t)32 << 20)) {
+    // Deferring means the array is read AFTER this call returns, which only page-locked memory makes worthwhile (an
+    // asynchronous copy from pageable memory blocks the host until it is staged: no overlap) and which a caller of a
+    // pageable buffer does not expect: such a buffer is copied during the call, as before.
+    bool pinned = false;
+    {
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, T_host) == cudaSuccess)
+            pinned = (at.type == cudaMemoryTypeHost || at.type == cudaMemoryTypeManaged);
+        else
+            cudaGetLastError();
+    }
+    if (pinned && !(per_member && ctx->g.batch > 1) && nzt >= 8 && bytes >= ((size_t)32 << 20)) {
         // deferred: the next shg_propagate enqueues the chunked copy (enqueue_upload) behind its own field uploads
         const int rc = shg_set_temperature(ctx, ctx->d_T_owned, T_uniform, per_member);
         ctx->up_host = T_host;
@@ -690,6 +674,9 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
             return SHG_EINVAL;
     }
     if (!ctx->T_set) return SHG_ESTATE;
+    // the paper's ordering (SHG_OPT_SCHEME = 1) exists with hi+lo constants and without heat output only; refused
+    // here, before anything is enqueued or any state of the last run is touched
+    if (ctx->scheme == 1 && (!ctx->precise || ctx->d_Q)) return SHG_EINVAL;
     if (!A1_in)                      // Gaussian pump of Eq. 6 / Eq. 5 from the beams of shg_create
         for (int b = 0; b < batch; ++b)
             if (!(ctx->beams[b].w0 > 0) || !(ctx->beams[b].P >= 0)) return SHG_EINVAL;
@@ -751,8 +738,13 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         if (k > g.nzt - 2) { k = g.nzt - 2; rem = g.nz; }
         return (int)(k + (rem != 0 ? 1 : 0));
     };
+    ctx->hist_valid = false;             // from here on the device history belongs to this run
     CU(cudaMemsetAsync(ctx->d_hfix, 0, sizeof(long long) * (size_t)g.batch * (ctx->nrec + 1) * 2, st));
-    CU(cudaMemsetAsync(ctx->d_barrier, 0, 8 * sizeof(unsigned int), st));
+    // barrier counters start at zero; the status word [1] is NOT cleared here: a timeout of an earlier propagate that
+    // nobody has synchronised on yet stays raised (this run's kernels then give up at their first barrier) until
+    // shg_synchronize / shg_power* has reported it
+    CU(cudaMemsetAsync(ctx->d_barrier, 0, sizeof(unsigned int), st));
+    CU(cudaMemsetAsync(ctx->d_barrier + 2, 0, 6 * sizeof(unsigned int), st));
     if (g.nzt > 0) CU(cudaMemsetAsync(ctx->d_phi, 0, sizeof(float) * (size_t)batch * np, st));
     {   // P_j(0) and the fixed-point scale of every member, from the input (before anything overwrites it)
         int ch = (int)(np / 4096);
@@ -857,7 +849,6 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         // The paper's ordering (Eq. 14-15): N(dz/2) - L(dz) - N(dz/2).  ROW_FIRST takes the first
         // half-step of step 0, the row pass n of the loop the second half of step n and the first half of step
         // n + 1, ROW_FINAL the second half of step nz - 1; every linear step is a full dz (tables 0).
-        if (!prec || P.Q) return SHG_EINVAL;     // this variant: hi+lo constants only, no heat output
         CU(wait_all_chunks());
         CU(ctx->Lx.row(P, shg::ROW_FIRST, 0, 0, prec, grid_r, st)); ++launches;
         CU(ctx->Ly.col(P, 0, prec, grid_c, st)); ++launches;
@@ -969,8 +960,11 @@ int shg_synchronize(shg_ctx* ctx) {
     unsigned int bs[2] = {0, 0};
     CU(cudaMemcpy(bs, ctx->d_barrier, sizeof(bs), cudaMemcpyDeviceToHost));
     if (bs[1] != 0) {
+        CU(cudaMemset(ctx->d_barrier + 1, 0, sizeof(unsigned int)));     // reported once, then cleared
+        ctx->hist_valid = false;
         g_cuda_msg = "persistent kernel: a device-wide barrier timed out (not all CTAs co-resident, or the spin limit "
-                     "of SHG_OPT_SPIN_LIMIT is too short for this run); the outputs of this propagate are invalid";
+                     "of SHG_OPT_SPIN_LIMIT is too short for this run); the outputs of every propagate enqueued since "
+                     "the last successful shg_synchronize / shg_power are invalid";
         return SHG_ECUDA;
     }
     return SHG_OK;
@@ -1082,43 +1076,6 @@ int shg_read_trace(shg_ctx* ctx, long long* out, int* steps, int* grid) {
     if (!ctx->d_trace || ctx->trace_grid == 0) return SHG_ESTATE;
     CU(cudaStreamSynchronize(ctx->last_stream));
     CU(cudaMemcpy(out, ctx->d_trace, sizeof(long long) * (size_t)(*steps) * ctx->trace_grid * 8, cudaMemcpyDeviceToHost));
-    return SHG_OK;
-}
-
-static int measure_fp32(double* tflops, bool distinct);
-
-int shg_measure_fp32_peak(double* tflops) { return measure_fp32(tflops, false); }
-int shg_measure_fp32_peak_distinct(double* tflops) { return measure_fp32(tflops, true); }
-
-static int measure_fp32(double* tflops, bool distinct) {
-    if (!tflops) return SHG_EINVAL;
-    int dev = 0, sms = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    float *out = nullptr, *in = nullptr;
-    CU(cudaMalloc((void**)&out, sizeof(float) * (size_t)sms * 512));
-    CU(cudaMalloc((void**)&in, 4096));
-    CU(cudaMemset(in, 0, 4096));
-    cudaEvent_t e0, e1;
-    CU(cudaEventCreate(&e0));
-    CU(cudaEventCreate(&e1));
-    const int iters = 20000;
-    float best = 0.f;
-    for (int rep = 0; rep < 4; ++rep) {        // first repetition warms up
-        CU(cudaEventRecord(e0, nullptr));
-        if (distinct) k_fp32_peak_distinct<<<sms, 512>>>(out, in, iters);
-        else k_fp32_peak<<<sms, 512>>>(out, in, iters);
-        CU(cudaEventRecord(e1, nullptr));
-        CU(cudaEventSynchronize(e1));
-        float ms = 0.f;
-        CU(cudaEventElapsedTime(&ms, e0, e1));
-        if (rep > 0 && (best == 0.f || ms < best)) best = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(out);
-    cudaFree(in);
-    *tflops = 2.0 * 16.0 * (double)iters * 512.0 * (double)sms / ((double)best * 1e-3) / 1e12;
     return SHG_OK;
 }
 

@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(CGeo<N, C>::THREADS, 1) k_cluster(Params P) {
     // Send the C blocks of a staging buffer: block d goes to slot `rank` of CTA d's receive buffer.  Called by ALL
     // warps once the owner warps have written the staging buffer (their generic-proxy writes fenced towards the async
     // proxy).  A warp issues its bulk copies one lane after the other (~60 clocks each: 16 copies from one warp
-    // cost ~1000 clocks, tests/probes/dsmem_alltoall.cu), so the C copies are spread over all warps of the CTA.
+    // cost ~1000 clocks, measured by a stand-alone probe: profiles/r02a_summary.md 7), so the C copies are spread over all warps of the CTA.
     auto send_blocks = [&](float2* xbuf, float2* recv, unsigned bar) {
         if (owner) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();

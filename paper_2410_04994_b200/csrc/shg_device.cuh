@@ -32,15 +32,6 @@
 
 namespace shg {
 
-// Build-time diagnostic (SHG_NVCC_EXTRA=-DSHG_WTRACE, not in the product build): lane 0 of every warp stamps the SM
-// clock at eight points of a row item of z-steps 100..163 into the tail of the SHG_OPT_TRACE buffer (run with
-// SHG_OPT_TRACE = 4096 and nz >= 4100; layout [64][grid][16 warps][8] after the first 200 x grid x 8 words).
-#ifdef SHG_WTRACE
-#define SHG_WT(i) do { if (wt && lane == 0) wt[i] = clock64(); } while (0)
-#else
-#define SHG_WT(i) do { } while (0)
-#endif
-
 template <int N> struct FftCfg;
 template <> struct FftCfg<64>   { static constexpr int R = 8,  M = 8;  };
 template <> struct FftCfg<128>  { static constexpr int R = 16, M = 8;  };
@@ -298,8 +289,9 @@ __device__ __forceinline__ PhaseCoef phase_coef(float c, float s, float k1, floa
 }
 
 // Uniform temperature (nzt == 0): phi(z) = dk z exactly (Eq. 3 with constant dk), so z-step n has the same three
-// sampled phases at every point.  They are reduced mod 2 pi in double and evaluated once per (member, step) into
-// the table ucoef[b][n][3] = {CA, CM, CB} as (u1x, u1y, u2x, u2y) (k_uniform_coefs, built with the other tables):
+// sampled phases at every point.  They are reduced mod 2 pi in double and evaluated once per step into
+// the table ucoef[n][3] = {CA, CM, CB} as (u1x, u1y, u2x, u2y) (k_uniform_coefs, built with the other tables; one
+// table for all members: kappa_j dz, dz and dk depend on the crystal and T_uniform only, not on a member's window):
 // the kernels read 48 bytes per item instead of repeating ~500 double-precision instructions.
 __device__ __forceinline__ void uniform_coefs(const MemberDev& mb, int n, PhaseCoef& CA, PhaseCoef& CM, PhaseCoef& CB) {
     const double TWO_PI = 6.283185307179586476925286766559;
@@ -319,7 +311,7 @@ __device__ __forceinline__ void uniform_coefs(const MemberDev& mb, int n, PhaseC
 }
 
 __device__ __forceinline__ void load_uniform_coefs(const Params& P, int b, int n, PhaseCoef& CA, PhaseCoef& CM, PhaseCoef& CB) {
-    const float4* uc = P.ucoef + ((size_t)b * P.nz + n) * 3;
+    const float4* uc = P.ucoef + (size_t)n * 3;        // the same for every member b (crystal and T_uniform only)
     const float4 a = __ldg(uc), c = __ldg(uc + 1), d = __ldg(uc + 2);
     CA.u1x = a.x; CA.u1y = a.y; CA.u2x = a.z; CA.u2y = a.w;
     CM.u1x = c.x; CM.u1y = c.y; CM.u2x = c.z; CM.u2y = c.w;
@@ -571,16 +563,12 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
     }
 
     if constexpr (MODE == ROW_MID) {
-#ifdef SHG_WTRACE
-        long long* wt = (P.trace && n >= 100 && n < 164) ? P.trace + 200 * (size_t)gridDim.x * 8 + (((size_t)(n - 100) * gridDim.x + blockIdx.x) * 16 + warp) * 8 : nullptr;
-#endif
-        SHG_WT(0);
         float2* A = (f ? P.A[1] : P.A[0]) + rbase;
         const float4* hx = P.hx[hsel] + ((size_t)b * 2 + f) * NX;
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = ldcg2(A + M * q + m);
         if constexpr (!TS) table_prefetch<R, M>(hx, m);
-        if (P.nzt == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.ucoef + ((size_t)b * P.nz + n) * 3));
+        if (P.nzt == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(P.ucoef + (size_t)n * 3));
         // temperature / phase operands of the first RK4 point are requested before the transform (when
         // registers allow), those of the second right after it; inside the loop two points ahead
         const size_t plane = (size_t)P.ny * NX;
@@ -597,9 +585,7 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             phi = P.phi + (size_t)b * plane + pbase;
             if constexpr (R < 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
         }
-        SHG_WT(1);
         warp_fft<NX, PREC>(v, own, tws, m);
-        SHG_WT(2);
         if (P.nzt != 0) {
             // (a 32-value line leaves no registers to carry operands across the transform)
             if constexpr (R >= 32) cur = t_load(Ta, Tn, plane, pbase, ta.two, tb.two, phi);
@@ -621,7 +607,6 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             for (int q = 0; q < R; ++q) own[M * q + m] = v[q];
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
-        SHG_WT(3);
 
         // ---- nonlinear step on elements e = M q + m + f N/2, q < R/2: own lower half, partner's upper half.
         // p1 / p2 address A1 / A2 of this lane's points whichever side it is on (no value selects).
@@ -757,7 +742,6 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             }
         }
         if constexpr (HEAT) { if (qrow) heat_half(false); }
-        SHG_WT(4);
         if (slot >= 0) {
             s1 = warp_sum_ll(s1); s2 = warp_sum_ll(s2);
             if (lane == 0) {
@@ -774,7 +758,6 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             }
         }
         if constexpr (G >= 2) __syncwarp(); else named_barrier(1 + (warp >> 1), 64);
-        SHG_WT(5);
         if constexpr (PK) {
 #pragma unroll
             for (int q = 0; q < R; q += 2) {
@@ -788,7 +771,6 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
         }
         __syncwarp();
         warp_fft<NX, PREC>(v, own, tws, m);
-        SHG_WT(6);
         if constexpr (TS)
             table_mul_s<R, M, PREC, false>(v, (unsigned)__cvta_generic_to_shared(stab + f * NX + m),
                                            std::make_integer_sequence<int, R>{});
@@ -796,7 +778,6 @@ __device__ __forceinline__ void row_item(const Params& P, const StepCtx& sc, int
             table_mul<R, M, PREC, false>(v, hx + m);
 #pragma unroll
         for (int q = 0; q < R; ++q) stcg2(A + M * q + m, v[q]);
-        SHG_WT(7);
     }
 }
 
@@ -1399,11 +1380,7 @@ __device__ __forceinline__ bool grid_barrier(const Params& P, unsigned int& epoc
         if (P.acquire_fence == 2) (void)ld_acquire_u32(P.barrier);
         else if (P.acquire_fence == 1) asm volatile("fence.acq_rel.gpu;" ::: "memory");
         ok = good;
-#ifdef SHG_WTRACE
-        if (P.trace != nullptr && n < (P.trace_steps < 200 ? P.trace_steps : 200)) {   // (the tail holds the warp stamps)
-#else
         if (P.trace != nullptr && n < P.trace_steps) {
-#endif
             long long* t = P.trace + (((size_t)n * gridDim.x + blockIdx.x) * 2 + which) * 4;
             unsigned long long gt;
             unsigned int smid;

@@ -43,7 +43,7 @@ struct Params {
     const float4* hx[2];       // [0]=full step dz, [1]=half step: [batch][2][nx]
     const float4* hy[2];       // [batch][2][ny], includes 1/(nx ny)
     const MemberDev* mem;      // [batch]
-    const float4* ucoef;       // nzt == 0: [batch][nz][3] coupling coefficients of every z-step (shg_device.cuh), else null
+    const float4* ucoef;       // nzt == 0: [nz][3] coupling coefficients of every z-step, shared by all members (shg_device.cuh), else null
     long long* hfix;           // [batch][nrec+1][2] power sums in fixed point: sum over points of rint(|A_j|^2 * pfix[b])
     const float* pfix;         // [batch] the member's fixed-point scale 2^e (k_input_power), see shg_device.cuh "power sums"
     float* Q;                  // optional heat-source output [batch][nq][ny][nx] (shg_set_heat_output), else null

@@ -21,9 +21,9 @@ OPT_SPIN_LIMIT, OPT_TABLES_SMEM, OPT_CLUSTER, OPT_PIPELINE = 7, 8, 9, 10
 
 EXPORTS = ("shg_create", "shg_set_option", "shg_set_temperature", "shg_set_temperature_host", "shg_propagate",
            "shg_propagate_host", "shg_set_heat_output", "shg_power", "shg_power_history", "shg_gaussian_input",
-           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace", "shg_measure_fp32_peak",
+           "shg_enable_timing", "shg_last_main_loop_ms", "shg_read_trace",
            "shg_last_launch_count", "shg_destroy", "shg_strerror", "shg_synchronize", "shg_history_length",
-           "shg_history_nodes", "shg_last_cluster_size", "shg_measure_fp32_peak_distinct", "shg_last_kernel",
+           "shg_history_nodes", "shg_last_cluster_size", "shg_last_kernel",
            "shg_field_power_static")
 
 
@@ -79,8 +79,6 @@ def lib():
     L.shg_last_cluster_size.argtypes = [vp]
     L.shg_last_kernel.argtypes = [vp]
     L.shg_set_heat_output.argtypes = [vp, vp, C.c_int]
-    L.shg_measure_fp32_peak.argtypes = [dp]
-    L.shg_measure_fp32_peak_distinct.argtypes = [dp]
     L.shg_field_power_static.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp, vp]
     L.shg_destroy.argtypes = [vp]
     L.shg_destroy.restype = None
@@ -119,20 +117,6 @@ def _dev_ptr(t, dtype_names):
     if str(t.dtype).replace("torch.", "") not in dtype_names:
         raise TypeError("expected dtype in %s, got %s" % (dtype_names, t.dtype))
     return C.c_void_p(t.data_ptr())
-
-
-def measure_fp32_peak() -> float:
-    """Measured fp32 FFMA peak of the current device in TFLOP/s (shg_measure_fp32_peak)."""
-    v = C.c_double()
-    _check(lib().shg_measure_fp32_peak(C.byref(v)))
-    return float(v.value)
-
-
-def measure_fp32_peak_distinct() -> float:
-    """The same with three distinct register operands per FFMA (shg_measure_fp32_peak_distinct)."""
-    v = C.c_double()
-    _check(lib().shg_measure_fp32_peak_distinct(C.byref(v)))
-    return float(v.value)
 
 
 def field_power_static(A1, A2, scale1: float, scale2: float, out, stream=None):

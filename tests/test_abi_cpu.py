@@ -31,6 +31,15 @@ def test_library_exports_every_declared_symbol(shg_mod):
     out = subprocess.run(["nm", "-D", "--defined-only", shg_mod.LIB_PATH], capture_output=True, text=True).stdout
     exported = set(re.findall(r" T (shg_[a-z_0-9]+)", out))
     assert declared <= exported
+    # the product library holds the method's calls only: bench.py's measuring equipment lives in libshg_diag
+    from paper_2410_04994_b200 import diag
+    hd = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "shg_diag.h")).read(), flags=re.S)
+    declared_diag = set(re.findall(r"\b(shg_[a-z_0-9]+)\s*\(", hd))
+    assert declared_diag == set(diag.EXPORTS) and not (declared_diag & exported)
+    out = subprocess.run(["nm", "-D", "--defined-only", diag.LIB_PATH], capture_output=True, text=True).stdout
+    assert declared_diag <= set(re.findall(r" T (shg_[a-z_0-9]+)", out))
+    for name in declared_diag:
+        assert hasattr(diag.lib(), name), name
 
 
 def test_argument_validation_and_no_cpu_fallback(shg_mod):

@@ -416,18 +416,26 @@ def test_overlapped_temperature_upload_gives_the_same_bits(name, nz):
     and shg_propagate launches the persistent kernel once per chunk, over the z-steps whose planes that chunk
     completes (k_persist for cfg5's 1 GiB array of 256 planes, k_persist_flat for cfg3's planes on the nodes): same
     fields and history as with the whole array resident on the device before the launch, also when the same context
-    propagates again without a new upload, and from pageable as well as pinned host memory."""
+    propagates again without a new upload.  Only page-locked memory is deferred: a pageable array is copied during
+    shg_set_temperature_host and may be overwritten or freed right after it."""
     w = wl.make(name, nz=nz)
     g1, g2, gh, cg = run_gpu(w)                                       # device-resident T: one launch of the z-loop
     assert cg.last_launch_count() == 5
     ctx = shg.Shg(w["grid"], w["crystal"], w["beams"])
     Tpin = torch.from_numpy(w["T"]).pin_memory()
-    for T in (Tpin, w["T"]):
-        ctx.set_temperature(T)                                        # host array -> chunked upload
+    for T, chunked in ((Tpin, True), (w["T"].copy(), False)):
+        ctx.set_temperature(T)                                        # pinned host array -> chunked upload by the propagate
+        if not chunked:
+            T[...] = np.nan                                           # a pageable array is copied during the call:
+            ctx._keep = []                                            # the caller may scribble over it or free it
+            del T
         A1 = torch.from_numpy(w["A1"]).cuda()
         h1, h2 = ctx.propagate(A1)
         ctx.synchronize()
-        assert ctx.last_launch_count() > 5 or nz < 40                 # several ranges (a 3-step run needs one chunk)
+        if chunked:
+            assert ctx.last_launch_count() > 5 or nz < 40             # several ranges (a 3-step run needs one chunk)
+        else:
+            assert ctx.last_launch_count() == 5
         assert np.array_equal(h1.cpu().numpy(), g1) and np.array_equal(h2.cpu().numpy(), g2)
         assert np.array_equal(ctx.power_history(0), gh[0])
     r1, r2 = ctx.propagate(A1)                                        # again, nothing pending: one launch
@@ -487,13 +495,14 @@ def test_argument_errors_on_device():
 
 @pytest.mark.parametrize("name,nz", [("cfg3", 60), ("cfg5", 8)])
 def test_barrier_acquire_modes_and_table_placement_are_bit_identical(name, nz):
-    """SHG_OPT_ACQUIRE_FENCE (ld.acquire poll = default / fence / none) and SHG_OPT_TABLES_SMEM only change how the
+    """SHG_OPT_ACQUIRE_FENCE (ld.acquire poll = default / fence) and SHG_OPT_TABLES_SMEM only change how the
     persistent kernel synchronises and where it reads its propagator tables from: same bits."""
     w = wl.make(name, nz=nz)
     a1, a2, ah, ca = run_gpu(w)
     assert ca.last_launch_count() == 5
-    for options in ({shg.OPT_ACQUIRE_FENCE: 1}, {shg.OPT_ACQUIRE_FENCE: 0}, {shg.OPT_TABLES_SMEM: 0},
-                    {shg.OPT_SPIN_LIMIT: 0}):
+    with pytest.raises(shg.ShgError):                      # the mode outside the memory model is not in the product
+        ca.set_option(shg.OPT_ACQUIRE_FENCE, 0)
+    for options in ({shg.OPT_ACQUIRE_FENCE: 1}, {shg.OPT_TABLES_SMEM: 0}, {shg.OPT_SPIN_LIMIT: 0}):
         b1, b2, bh, _ = run_gpu(w, options=options)
         assert np.array_equal(a1, b1) and np.array_equal(a2, b2) and np.array_equal(ah[0], bh[0]), options
 
@@ -731,8 +740,15 @@ def test_paper_ordering_launch_schemes_agree_and_argument_errors():
     assert ca.last_launch_count() == 5 and cb.last_launch_count() == 4 + 2 * (20 - 1)
     assert np.array_equal(a1, b1) and np.array_equal(a2, b2)
     ca.set_option(shg.OPT_PRECISE, 0)
-    with pytest.raises(shg.ShgError):
-        ca.propagate(torch.from_numpy(w["A1"]).cuda())
+    # refused before anything is enqueued: the outputs are untouched and shg_power still describes the run before
+    o1 = torch.full((1, 128, 128), 7.0 + 0j, dtype=torch.complex64, device="cuda")
+    o2 = o1.clone()
+    with pytest.raises(shg.ShgError) as err:
+        ca.propagate(torch.from_numpy(w["A1"]).cuda(), None, o1, o2)
+    assert err.value.code == shg.SHG_EINVAL
+    torch.cuda.synchronize()
+    assert bool((o1 == 7.0).all()) and bool((o2 == 7.0).all())
+    assert np.array_equal(ca.power_history(0), ah[0])
     with pytest.raises(shg.ShgError):
         ca.set_option(shg.OPT_SCHEME, 2)
 
