@@ -147,6 +147,10 @@ int shg_create(const shg_grid* grid, const shg_crystal* crystal, const shg_beam*
 int shg_set_option(shg_ctx* ctx, int option, int value);
 
 /* Temperature field.  nzt == 0: T is ignored (may be NULL) and every point has temperature T_uniform.
+ * A new T_uniform alone costs two small kernels at the head of the next shg_propagate, on that call's stream: no host
+ * copy and no host wait, so a sweep over T_uniform enqueues propagate after propagate without synchronising.
+ * (shg_set_option(SHG_OPT_UNDEPLETED | SHG_OPT_PRECISE) rebuilds all tables: the next propagate then waits for the
+ * context's last one and uploads them with blocking copies.)
  * nzt >= 1: T is a DEVICE fp32 array [per_member ? batch : 1][nzt][ny][nx]; it is BORROWED (not copied)
  * and must stay valid and unchanged until every propagate that uses it has completed. */
 int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, int per_member);

@@ -147,6 +147,13 @@ __global__ void k_uniform_coefs(const shg::MemberDev* mem, float4* ucoef, int nz
     ucoef[(size_t)i * 3 + 2] = make_float4(d.u1x, d.u1y, d.u2x, d.u2y);
 }
 
+// A new uniform temperature changes one scalar per member, dk_uniform = dk0 + ddk_dT (T_uniform - T_pm) (Eq. 3):
+// written on the propagate's stream, so that a sweep over T_uniform needs neither a host copy nor a host wait.
+__global__ void k_set_dk_uniform(shg::MemberDev* mem, int batch, double dk) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) mem[b].dk_uniform = dk;
+}
+
 }  // namespace
 
 struct shg_ctx {
@@ -166,6 +173,7 @@ struct shg_ctx {
     bool undepleted = false;
     int scheme = 0;
     bool tables_dirty = true;
+    bool uniform_dirty = false;           // only T_uniform changed since the tables were built (k_set_dk_uniform)
 
     Launchers Lx{}, Ly{};
 
@@ -342,6 +350,7 @@ int upload_tables(shg_ctx* ctx) {
         CU(cudaStreamSynchronize(nullptr));
     }
     ctx->tables_dirty = false;
+    ctx->uniform_dirty = false;
     return SHG_OK;
 }
 
@@ -540,7 +549,7 @@ int shg_set_temperature(shg_ctx* ctx, const float* T_device, double T_uniform, i
     if (ctx->g.nzt > 0 && (!T_device || !aligned16(T_device))) return SHG_EINVAL;
     ctx->d_T = (ctx->g.nzt > 0) ? T_device : nullptr;
     ctx->T_per_member = per_member ? 1 : 0;
-    if (ctx->T_uniform != T_uniform) { ctx->T_uniform = T_uniform; ctx->tables_dirty = true; }
+    if (ctx->T_uniform != T_uniform) { ctx->T_uniform = T_uniform; ctx->uniform_dirty = true; }
     ctx->T_set = true;
     if (T_device != ctx->d_T_owned) { ctx->up_chunks = 0; ctx->up_host = nullptr; }
     return SHG_OK;
@@ -686,6 +695,24 @@ int shg_propagate(shg_ctx* ctx, const void* A1_in, const void* A2_in, void* A1_o
         CU(cudaStreamSynchronize(ctx->last_stream));
         int rc = upload_tables(ctx);
         if (rc != SHG_OK) return rc;
+    }
+    if (ctx->uniform_dirty) {
+        // Only T_uniform changed: two small kernels on this propagate's stream, no copy, no host wait (a sweep over
+        // T_uniform enqueues and returns).  A propagate still running on ANOTHER stream reads the same scalars: this
+        // stream waits for it on the device.
+        if (ctx->last_batch != 0 && ctx->last_stream != st) {
+            if (!ctx->guard_ev) CU(cudaEventCreateWithFlags(&ctx->guard_ev, cudaEventDisableTiming));
+            CU(cudaEventRecord(ctx->guard_ev, ctx->last_stream));
+            CU(cudaStreamWaitEvent(st, ctx->guard_ev, 0));
+        }
+        const double dk = ctx->c.dk0 + ctx->c.ddk_dT * (ctx->T_uniform - ctx->c.T_pm);
+        k_set_dk_uniform<<<(ctx->g.batch + 127) / 128, 128, 0, st>>>(ctx->d_mem, ctx->g.batch, dk);
+        CU(cudaGetLastError());
+        if (ctx->d_ucoef) {
+            k_uniform_coefs<<<(ctx->g.nz + 127) / 128, 128, 0, st>>>(ctx->d_mem, ctx->d_ucoef, ctx->g.nz);
+            CU(cudaGetLastError());
+        }
+        ctx->uniform_dirty = false;
     }
     if (!A1_in) {
         int rc = shg_gaussian_input(ctx, A1_out, batch, cuda_stream);

@@ -445,6 +445,49 @@ def test_overlapped_temperature_upload_gives_the_same_bits(name, nz):
     ctx.close()
 
 
+def test_uniform_temperature_sweep_enqueues_without_a_host_wait():
+    """A sweep over T_uniform on one context: every shg_set_temperature + shg_propagate returns while the stream is
+    still held up by earlier work (no hidden synchronisation, no blocking table upload), and the last run of the sweep
+    has the bits of a fresh context created for that temperature."""
+    import time
+    w = wl.make("cfg1", nz=50)
+    c = dict(w["crystal"], ddk_dT=-300.0)
+    temps = [wl.T_PM + 0.25 * k for k in range(1, 9)]
+    ctx = shg.Shg(w["grid"], c, w["beams"])
+    ctx.set_temperature(None, wl.T_PM)
+    A1 = torch.from_numpy(w["A1"]).cuda()
+    o1, o2 = ctx.propagate(A1)                                 # warm-up: modules loaded, buffers allocated
+    ctx.synchronize()
+    etas = []
+    torch.cuda.synchronize()
+    done = torch.cuda.Event()
+    torch.cuda._sleep(2_000_000_000)                           # ~1 s of GPU time at the head of the stream
+    t0 = time.perf_counter()
+    for T in temps:
+        ctx.set_temperature(None, T)
+        ctx.propagate(A1, None, o1, o2)
+    host_s = time.perf_counter() - t0
+    done.record()
+    still_busy = not done.query()
+    torch.cuda.synchronize()
+    assert still_busy and host_s < 0.5, "the sweep waited for the device (%.3f s on the host)" % host_s
+    ctx.synchronize()
+    hist = ctx.power_history(0)
+    fresh = shg.Shg(w["grid"], c, w["beams"])
+    fresh.set_temperature(None, temps[-1])
+    f1, f2 = fresh.propagate(A1)
+    fresh.synchronize()
+    assert np.array_equal(o1.cpu().numpy(), f1.cpu().numpy()) and np.array_equal(o2.cpu().numpy(), f2.cpu().numpy())
+    assert np.array_equal(hist, fresh.power_history(0))
+    # and the temperature matters: the detuned run converts less than the phase-matched one
+    pm = shg.Shg(w["grid"], c, w["beams"])
+    pm.set_temperature(None, wl.T_PM)
+    pm.propagate(A1)
+    assert fresh.efficiency(0) < 0.9 * pm.efficiency(0)
+    for x in (ctx, fresh, pm):
+        x.close()
+
+
 def test_precise_constants_matter_over_many_steps():
     """with plain fp32 constants the error grows linearly with the step count; the hi+lo
     constants keep cfg2 (1000 steps) well inside the tolerance."""
