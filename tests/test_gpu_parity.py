@@ -139,7 +139,8 @@ def test_cfg5_reduced_length_elementwise():
 def test_cfg5_full_length_against_the_stored_oracle_run():
     """The full 10 000-step stress run in the launch configuration bench.py times, against the oracle's run of the
     same config stored by tests/golden/make_cfg5_golden.py (oracle only, ~30 min on 8 cores): relative L2 of
-    both output fields over the stored 256 x 256 sub-lattice (<= 2e-4, the north_star bar), every one of the
+    both output fields over a stored uniform random sample of 65 536 grid points (<= 2e-4, the north_star bar), the
+    power of each of the 256 tiles of 64 x 64 points (<= 1e-4 of the total: every point is in one), every one of the
     10 001 history nodes, the efficiency; plus what holds at any size (power books, finiteness)."""
     w = wl.make("cfg5")
     g1, g2, gh, ctx = run_gpu(w)
@@ -156,21 +157,29 @@ def test_cfg5_full_length_against_the_stored_oracle_run():
     import json, os
     gdir = os.path.join(os.path.dirname(__file__), "golden")
     G = json.load(open(os.path.join(gdir, "cfg5_oracle_summary.json")))
-    lat = np.load(os.path.join(gdir, "cfg5_oracle_lattice.npz"))
+    smp = np.load(os.path.join(gdir, "cfg5_oracle_sample.npz"))
     assert G["nz"] == 10000 and G["nx"] == 1024
     assert abs(eta / G["eta"] - 1) <= TOL_ETA
     assert abs(h[-1, 0] / G["P1_L"] - 1) <= TOL_ETA
-    oy, ox, st = int(lat["oy"]), int(lat["ox"]), int(lat["stride"])
-    for name, gf, of in (("A1", g1[0], lat["A1"]), ("A2", g2[0], lat["A2"])):
-        sub = gf[oy::st, ox::st]
-        assert sub.shape == of.shape == (256, 256)
+    # 65 536 distinct points drawn uniformly from the whole grid: every lane (ix mod 32), strip column (ix mod 8)
+    # and register index of the kernels' data layout is in the compared set
+    idx, tile = smp["idx"].astype(np.int64), int(smp["tile"])
+    assert idx.size == np.unique(idx).size == 65536
+    assert np.unique((idx % 1024) % 32).size == 32 and np.unique((idx // 1024) % 32).size == 32
+    for name, gf, of, ot in (("A1", g1[0], smp["A1"], smp["tiles1"]), ("A2", g2[0], smp["A2"], smp["tiles2"])):
+        sub = gf.ravel()[idx]
         e = rel_l2(sub, of)
-        print("cfg5 full length: %s rel-L2 over the lattice %.3e" % (name, e))
-        assert e <= TOL_FIELD, "%s rel-L2 over the lattice %.3e" % (name, e)
+        print("cfg5 full length: %s rel-L2 over the sample %.3e" % (name, e))
+        assert e <= TOL_FIELD, "%s rel-L2 over the sample %.3e" % (name, e)
         assert np.max(np.abs(sub - of)) <= 10 * TOL_FIELD * np.max(np.abs(of))
-        # the lattice carries its share of the field: its norm matches the stored full-field norm
-        assert abs(np.linalg.norm(of.astype(np.complex128)) * st / G[name + "_l2"] - 1) < 0.02
-    ho = lat["history"]
+        # the sample carries its share of the field: 1/16 of the points, 1/16 of the stored full-field power
+        assert abs(np.linalg.norm(of.astype(np.complex128)) * 4 / G[name + "_l2"] - 1) < 0.02
+        # ... and EVERY point enters the power of its 64 x 64 tile: 256 tile powers per field against the oracle's
+        gt = (np.abs(gf.astype(np.complex128)) ** 2).reshape(1024 // tile, tile, 1024 // tile, tile).sum(axis=(1, 3))
+        dev = np.max(np.abs(gt - ot)) / ot.sum()
+        print("cfg5 full length: %s tile powers max dev %.3e of the total" % (name, dev))
+        assert gt.shape == ot.shape == (16, 16) and dev <= TOL_ETA
+    ho = smp["history"]
     assert ho.shape == h.shape == (10001, 2)
     p0 = ho[0, 0] + ho[0, 1]
     print("cfg5 full length: history max dev %.3e / %.3e of P(0)" % (np.max(np.abs(h[:, 0] - ho[:, 0])) / p0,
